@@ -1,0 +1,122 @@
+/*
+ * mdwf.h -- C ABI of the B200-native Moebius domain-wall fermion (MDWF) solver library.
+ *
+ * The library computes the hot path of arXiv:1701.07559 (PAPER.md = the paper's text):
+ * the valence MDWF inversion, i.e. the 4D even-odd ("asymmetric", Sec. VII)
+ * Schur-preconditioned 5D Moebius operator built from the Moebius kernel of Eq. (2)
+ * (parameters M5, L5, b5, c5 of Table II), applied inside
+ * a mixed-precision ("double-half") conjugate-gradient solve on the normal
+ * equations.  It plays the role of the Chroma<->QUDA solver interface of PAPER.md:350.
+ *
+ * Operator (the paper cites [113-115] for it and does not print it):
+ *   D    = A - (1/2) H B,  A = alpha + beta Lambda,  B = b5 + c5 Lambda,
+ *          alpha = b5 (4 - M5) + 1, beta = c5 (4 - M5) - 1,
+ *          H = 4D Wilson hopping term (periodic x,y,z; antiperiodic t, applied in-kernel),
+ *          (Lambda psi)_s = P- psi_{s+1} + P+ psi_{s-1} with the -m_f wall factor at the wrap.
+ *   Mpc  = A - (1/4) H_oe B A^{-1} H_eo B  on odd sites (odd = (x+y+z+t) & 1 == 1).
+ *
+ * Conventions
+ *   - All pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The caller owns
+ *     every buffer it passes; the library copies what it needs and never keeps caller pointers.
+ *   - real_bytes is 8 (double) or 4 (float): the type of the caller's buffer.  Complex numbers
+ *     are interleaved (re, im).  Arrays are C-ordered:
+ *       gauge          U[t][z][y][x][mu][row][col], mu in {x,y,z,t}; U_mu(x) is the link from x to
+ *                      x+mu; plain SU(3), no boundary sign folded in.        (4 V4 x 18 reals)
+ *       5D spinor      psi[s][t][z][y][x][spin][colour]                      (L5 V4 x 24 reals)
+ *       parity spinor  psi[s][cb][spin][colour], cb = lex(x,y,z,t)/2 over the ODD sites,
+ *                      lex = x + Lx (y + Ly (z + Lz t)).                     (L5 V4/2 x 24 reals)
+ *     gamma matrices: DeGrand-Rossi basis, gamma5 = diag(+1,+1,-1,-1).
+ *   - All work is enqueued on the context's stream (option "stream", default: the legacy default
+ *     stream).  Functions that return scalars synchronise that stream before returning.
+ *   - Every function returns MDWF_OK (0) or a negative error code; mdwf_last_error() gives text.
+ *     There is no CPU fallback: without a CUDA device every compute call returns MDWF_ECUDA.
+ */
+#ifndef MDWF_H
+#define MDWF_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mdwf_ctx mdwf_ctx; /* opaque, owned by the library */
+
+enum {
+    MDWF_OK = 0,
+    MDWF_EARG = -1,     /* bad argument: odd extent, L5 < 2 or > 32, null pointer, bad real_bytes/op/option */
+    MDWF_ENOGAUGE = -2, /* gauge field not loaded */
+    MDWF_ECUDA = -3,    /* CUDA error (text in mdwf_last_error) */
+    MDWF_ENOCONV = -4,  /* solver did not reach tol within maxiter; sol holds the best iterate */
+    MDWF_ENOMEM = -5    /* device allocation failed */
+};
+
+enum { /* op codes of mdwf_apply */
+    MDWF_OP_MPC = 0,       /* Mpc        : parity spinor -> parity spinor (S5 of the hot path)   */
+    MDWF_OP_MPCDAG = 1,    /* Mpc^dagger : parity spinor -> parity spinor (S6)                   */
+    MDWF_OP_MDAGM = 2,     /* Mpc^dagger Mpc                                                   */
+    MDWF_OP_D = 3,         /* D          : full 5D spinor -> full 5D spinor                     */
+    MDWF_OP_DDAG = 4       /* D^dagger                                                          */
+};
+
+/* Create a context for an Lx x Ly x Lz x Lt x L5 lattice (all 4D extents even, 2 <= L5 <= 32) and the
+ * Moebius parameters of Eq. (2) / Table II.  Precomputes alpha, beta and the fifth-dimension tables. */
+int mdwf_create(mdwf_ctx **out, int Lx, int Ly, int Lz, int Lt, int L5,
+                double M5, double b5, double c5, double m_f);
+int mdwf_destroy(mdwf_ctx *ctx);
+
+/* Options (key, value as strings):
+ *   "ladder"          "d" | "ds" | "dh" | "dsh"   precision ladder of mdwf_solve: fp64 only; fp64 reliable
+ *                     updates + fp32 sloppy; fp64 + 16-bit sloppy; fp64 reliable residual + fp32 solution
+ *                     accumulator + 16-bit operator and Krylov vectors ("double/single/half").  Default "d".
+ *   "apply_precision" "auto" | "fp64" | "fp32" | "half"   arithmetic/storage used inside mdwf_apply;
+ *                     "auto" = that of the caller's buffer (real_bytes).  Default "auto".
+ *   "reconstruct"     "18" | "12"   SU(3) link storage; 12 keeps rows 0,1 and rebuilds row 2 =
+ *                     conj(row0 x row1) in-kernel.  Takes effect at the next mdwf_load_gauge.  Default "18".
+ *   "reliable_delta"  reliable-update threshold delta (default "0.1").
+ *   "stream"          cudaStream_t as a decimal integer (default "0").
+ *   "matpc"           "asym" only (the operator Chroma uses).
+ */
+int mdwf_set_option(mdwf_ctx *ctx, const char *key, const char *value);
+
+/* Copy the gauge field into the library's even-odd device layouts (fp64, fp32 and 16-bit copies). */
+int mdwf_load_gauge(mdwf_ctx *ctx, const void *U_dev, int real_bytes);
+int mdwf_load_gauge_host(mdwf_ctx *ctx, const void *U_host, int real_bytes);
+
+/* out = op(in).  ops 0-2: parity spinors (odd sites); ops 3-4: full 5D spinors.  in_dev != out_dev. */
+int mdwf_apply(mdwf_ctx *ctx, int op, const void *in_dev, void *out_dev, int real_bytes);
+
+/* Solve D x = src on the full 5D lattice (fp64 buffers): Schur preparation b' = b_o - D_oe A^{-1} b_e,
+ * CG on Mpc^dagger Mpc (CGLS recurrences) with the configured precision ladder and reliable updates,
+ * reconstruction x_e = A^{-1}(b_e - D_eo x_o).  tol is the target for ||src - D x|| / ||src||.
+ * iters_out = CG iterations (one Mpc + one Mpc^dagger each); true_res_out = ||src - D x||_2 / ||src||_2
+ * recomputed in fp64 with the unpreconditioned operator.  Returns MDWF_ENOCONV if maxiter was hit. */
+int mdwf_solve(mdwf_ctx *ctx, const void *src_dev, void *sol_dev, double tol, int maxiter,
+               int *iters_out, double *true_res_out);
+/* Same with HOST buffers (fp64): host->device copy of src and device->host copy of sol included. */
+int mdwf_solve_host(mdwf_ctx *ctx, const void *src_host, void *sol_host, double tol, int maxiter,
+                    int *iters_out, double *true_res_out);
+
+/* Deterministic BLAS-1 (S7) on flat device arrays of n reals (real_bytes 8 or 4); fp64 accumulation,
+ * fixed reduction order (per-thread strided sums, warp shuffles, block tree, fixed-order final pass). */
+int mdwf_blas_norm2(mdwf_ctx *ctx, const void *x_dev, long long n, int real_bytes, double *out);
+int mdwf_blas_redot(mdwf_ctx *ctx, const void *x_dev, const void *y_dev, long long n, int real_bytes, double *out);
+int mdwf_blas_axpy(mdwf_ctx *ctx, double a, const void *x_dev, void *y_dev, long long n, int real_bytes);
+
+/* Per-context counters.  Keys: "launches" (kernels launched so far), "iterations", "reliable_updates",
+ * "solve_seconds" (device time of the last solve, CUDA events), "true_residual", "op_applications"
+ * (Mpc + Mpc^dagger applications in the last solve, all precisions), "sloppy_applications". */
+int mdwf_get_stat(const mdwf_ctx *ctx, const char *key, double *value);
+
+/* Measurement: run op (MDWF_OP_MPC or MDWF_OP_MPCDAG) `reps` times after `warmup`
+ * untimed runs, in precision "fp64" | "fp32" | "half", on library-owned hash-filled vectors, timed with
+ * CUDA events on the context's stream.  out4[0] = ms per application (both kernels), out4[1] / out4[2] =
+ * ms per launch of its first / second kernel timed alone, out4[3] = kernels launched by this call. */
+int mdwf_time_op(mdwf_ctx *ctx, int op, const char *precision, int reps, int warmup, double *out4);
+
+const char *mdwf_last_error(const mdwf_ctx *ctx);
+/* The fixed flop count per odd 5D site per Mpc application: 2880 + 48 L5. */
+int mdwf_flops_per_site(const mdwf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MDWF_H */

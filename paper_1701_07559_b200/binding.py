@@ -1,0 +1,187 @@
+"""Thin ctypes binding of include/mdwf.h: same names, argument marshalling only.
+
+PyTorch appears here only as the owner of device memory (tensor.data_ptr()) and streams.
+There is no CPU fallback: lib() raises if libmdwf_b200.so has not been built, and every compute
+call returns the library's error code (raised as MdwfError) when no CUDA device is present.
+"""
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmdwf_b200.so")
+
+MDWF_OK, MDWF_EARG, MDWF_ENOGAUGE, MDWF_ECUDA, MDWF_ENOCONV, MDWF_ENOMEM = 0, -1, -2, -3, -4, -5
+OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG = 0, 1, 2, 3, 4
+
+EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
+           "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
+           "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op"]
+
+_lib = None
+
+
+class MdwfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("mdwf error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib():
+    """Load the C-ABI library; fail loudly if it is missing (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libmdwf_b200.so is not built: run `python -m paper_1701_07559_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        P, I, D, LL = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
+        L.mdwf_create.argtypes = [ctypes.POINTER(P), I, I, I, I, I, D, D, D, D]
+        L.mdwf_destroy.argtypes = [P]
+        L.mdwf_set_option.argtypes = [P, ctypes.c_char_p, ctypes.c_char_p]
+        L.mdwf_load_gauge.argtypes = [P, P, I]
+        L.mdwf_load_gauge_host.argtypes = [P, P, I]
+        L.mdwf_apply.argtypes = [P, I, P, P, I]
+        L.mdwf_solve.argtypes = [P, P, P, D, I, ctypes.POINTER(I), ctypes.POINTER(D)]
+        L.mdwf_solve_host.argtypes = [P, P, P, D, I, ctypes.POINTER(I), ctypes.POINTER(D)]
+        L.mdwf_blas_norm2.argtypes = [P, P, LL, I, ctypes.POINTER(D)]
+        L.mdwf_blas_redot.argtypes = [P, P, P, LL, I, ctypes.POINTER(D)]
+        L.mdwf_blas_axpy.argtypes = [P, D, P, P, LL, I]
+        L.mdwf_get_stat.argtypes = [P, ctypes.c_char_p, ctypes.POINTER(D)]
+        L.mdwf_last_error.argtypes = [P]
+        L.mdwf_last_error.restype = ctypes.c_char_p
+        L.mdwf_flops_per_site.argtypes = [P]
+        L.mdwf_time_op.argtypes = [P, I, ctypes.c_char_p, I, I, ctypes.POINTER(D)]
+        _lib = L
+    return _lib
+
+
+# ---- same-name functions on raw pointers / integers ---------------------------------------------
+def mdwf_create(Lx, Ly, Lz, Lt, L5, M5, b5, c5, m_f):
+    h = ctypes.c_void_p()
+    rc = lib().mdwf_create(ctypes.byref(h), Lx, Ly, Lz, Lt, L5, M5, b5, c5, m_f)
+    if rc != MDWF_OK:
+        raise MdwfError(rc, "mdwf_create: bad argument")
+    return h
+
+
+def _check(h, rc, allow=()):
+    if rc != MDWF_OK and rc not in allow:
+        raise MdwfError(rc, lib().mdwf_last_error(h).decode())
+    return rc
+
+
+def mdwf_destroy(h):
+    return lib().mdwf_destroy(h)
+
+
+def mdwf_set_option(h, key, value):
+    return _check(h, lib().mdwf_set_option(h, key.encode(), str(value).encode()))
+
+
+def mdwf_load_gauge(h, U_ptr, real_bytes):
+    return _check(h, lib().mdwf_load_gauge(h, U_ptr, real_bytes))
+
+
+def mdwf_load_gauge_host(h, U_ptr, real_bytes):
+    return _check(h, lib().mdwf_load_gauge_host(h, U_ptr, real_bytes))
+
+
+def mdwf_apply(h, op, in_ptr, out_ptr, real_bytes):
+    return _check(h, lib().mdwf_apply(h, op, in_ptr, out_ptr, real_bytes))
+
+
+def mdwf_solve(h, src_ptr, sol_ptr, tol, maxiter, host=False):
+    it, tr = ctypes.c_int(0), ctypes.c_double(0.0)
+    fn = lib().mdwf_solve_host if host else lib().mdwf_solve
+    rc = _check(h, fn(h, src_ptr, sol_ptr, tol, maxiter, ctypes.byref(it), ctypes.byref(tr)), allow=(MDWF_ENOCONV,))
+    return rc, it.value, tr.value
+
+
+def mdwf_get_stat(h, key):
+    v = ctypes.c_double(0.0)
+    _check(h, lib().mdwf_get_stat(h, key.encode(), ctypes.byref(v)))
+    return v.value
+
+
+def mdwf_flops_per_site(h):
+    return lib().mdwf_flops_per_site(h)
+
+
+def mdwf_time_op(h, op, precision, reps, warmup):
+    """Average device milliseconds per application (CUDA events on the context's stream) of op
+    0 Mpc / 1 Mpc^dagger in the given precision on library-owned buffers; also per-kernel times."""
+    out = (ctypes.c_double * 4)()
+    _check(h, lib().mdwf_time_op(h, op, precision.encode(), reps, warmup, out))
+    return dict(ms=out[0], ms_k1=out[1], ms_k2=out[2], launches=out[3])
+
+
+# ---- convenience wrapper on torch tensors (marshalling only) ------------------------------------
+class Mdwf:
+    def __init__(self, L, L5, M5, b5, c5, mf):
+        self.L, self.L5 = tuple(L), L5
+        self.h = mdwf_create(L[0], L[1], L[2], L[3], L5, M5, b5, c5, mf)
+
+    def close(self):
+        if self.h is not None:
+            mdwf_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key, value):
+        mdwf_set_option(self.h, key, value)
+
+    @staticmethod
+    def _rb(t):
+        import torch
+        return 8 if t.dtype in (torch.complex128, torch.float64) else 4
+
+    def load_gauge(self, U):
+        assert U.is_contiguous()
+        if U.is_cuda:
+            mdwf_load_gauge(self.h, U.data_ptr(), self._rb(U))
+        else:
+            mdwf_load_gauge_host(self.h, U.data_ptr(), self._rb(U))
+
+    def apply(self, op, x):
+        import torch
+        assert x.is_cuda and x.is_contiguous()
+        out = torch.empty_like(x)
+        mdwf_apply(self.h, op, x.data_ptr(), out.data_ptr(), self._rb(x))
+        return out
+
+    def solve(self, src, tol=1e-10, maxiter=20000):
+        import torch
+        assert src.is_contiguous() and src.dtype == torch.complex128
+        sol = torch.empty_like(src)
+        rc, it, tr = mdwf_solve(self.h, src.data_ptr(), sol.data_ptr(), tol, maxiter, host=not src.is_cuda)
+        return sol, it, tr, rc
+
+    def stat(self, key):
+        return mdwf_get_stat(self.h, key)
+
+    def flops_per_site(self):
+        return mdwf_flops_per_site(self.h)
+
+    def time_op(self, op, precision, reps=20, warmup=3):
+        return mdwf_time_op(self.h, op, precision, reps, warmup)
+
+    def norm2(self, x):
+        v = ctypes.c_double(0.0)
+        n = x.numel() * (2 if x.is_complex() else 1)
+        _check(self.h, lib().mdwf_blas_norm2(self.h, x.data_ptr(), n, self._rb(x), ctypes.byref(v)))
+        return v.value
+
+    def redot(self, x, y):
+        v = ctypes.c_double(0.0)
+        n = x.numel() * (2 if x.is_complex() else 1)
+        _check(self.h, lib().mdwf_blas_redot(self.h, x.data_ptr(), y.data_ptr(), n, self._rb(x), ctypes.byref(v)))
+        return v.value
+
+    def axpy(self, a, x, y):
+        n = x.numel() * (2 if x.is_complex() else 1)
+        _check(self.h, lib().mdwf_blas_axpy(self.h, float(a), x.data_ptr(), y.data_ptr(), n, self._rb(x)))

@@ -1,0 +1,236 @@
+// blas_kernels.cu -- deterministic BLAS-1 (S7) on device-layout parity vectors and on flat arrays.
+//
+// Determinism: every thread accumulates a fixed set of elements in fp64, a warp is reduced with a fixed
+// xor-shuffle tree, a block with a fixed tree over its warps, each block writes ONE partial to
+// partial[blockIdx.x] and a single-block second kernel adds the partials in a fixed strided order.
+// The grid is a pure function of the problem size, so results are bit-reproducible run to run.
+// No floating-point atomics anywhere.
+#include "mdwf_device.cuh"
+#include "mdwf_internal.h"
+
+#define RED_THREADS 256
+#define RED_MAX_BLOCKS 4096
+
+int mdwf_reduce_max_blocks() { return RED_MAX_BLOCKS; }
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void block_partial(double v, double *partial)
+{
+    __shared__ double wsum[RED_THREADS / 32];
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wsum[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        double t = (lane < RED_THREADS / 32) ? wsum[lane] : 0.0;
+        t = warp_sum(t);
+        if (lane == 0) partial[blockIdx.x] = t;
+    }
+}
+
+__global__ void final_sum_kernel(const double *partial, int n, double *result)
+{
+    double v = 0.0;
+    for (int i = threadIdx.x; i < n; i += RED_THREADS) v += partial[i];
+    __shared__ double wsum[RED_THREADS / 32];
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wsum[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        double t = (lane < RED_THREADS / 32) ? wsum[lane] : 0.0;
+        t = warp_sum(t);
+        if (lane == 0) *result = t;
+    }
+}
+
+static int red_blocks(long long work)
+{
+    long long b = (work + RED_THREADS - 1) / RED_THREADS;
+    if (b > RED_MAX_BLOCKS) b = RED_MAX_BLOCKS;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+// ---- parity vectors: out = a x + b y  (+ ||out||^2) -------------------------------------------
+template <class PO, class PX, class PY, bool HASY, bool NORM>
+__global__ void __launch_bounds__(RED_THREADS)
+axpby_kernel(void *out, float *out_norm, double a, const void *x, const float *xn, double b, const void *y,
+             const float *yn, int L5, long Vh, double *partial)
+{
+    using RO = typename PO::R;
+    const long n5 = (long)L5 * Vh;
+    double sum = 0.0;
+    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
+        const int s = (int)(idx / Vh);
+        const long cb = idx - (long)s * Vh;
+        typename PX::R vx[24];
+        load_spinor<PX>(x, xn, s, cb, Vh, vx);
+        RO r[24];
+        if (HASY) {
+            typename PY::R vy[24];
+            load_spinor<PY>(y, yn, s, cb, Vh, vy);
+#pragma unroll
+            for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k] + b * (double)vy[k]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k]);
+        }
+        store_spinor<PO>(out, out_norm, s, cb, Vh, r);
+        if (NORM) {
+#pragma unroll
+            for (int k = 0; k < 24; k++) sum += (double)r[k] * (double)r[k];
+        }
+    }
+    if (NORM) block_partial(sum, partial);
+}
+
+template <class PX, class PY, int KIND>
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_kernel(const void *x, const float *xn, const void *y, const float *yn, int L5, long Vh, double *partial)
+{
+    const long n5 = (long)L5 * Vh;
+    double sum = 0.0;
+    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
+        const int s = (int)(idx / Vh);
+        const long cb = idx - (long)s * Vh;
+        typename PX::R vx[24];
+        load_spinor<PX>(x, xn, s, cb, Vh, vx);
+        if (KIND == 0) {
+#pragma unroll
+            for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vx[k];
+        } else {
+            typename PY::R vy[24];
+            load_spinor<PY>(y, yn, s, cb, Vh, vy);
+#pragma unroll
+            for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vy[k];
+        }
+    }
+    block_partial(sum, partial);
+}
+
+template <class PO, class PX, class PY>
+static int axpby_xy(const SpinorBuf &out, double a, const SpinorBuf &x, double b, const SpinorBuf &y, int L5, int Vh,
+                    double *partial, double *result, cudaStream_t st)
+{
+    const int nb = red_blocks((long long)L5 * Vh);
+    const bool hasy = (y.v != nullptr);
+    const bool norm = (partial != nullptr);
+#define AX(HY, NM) axpby_kernel<PO, PX, PY, HY, NM><<<nb, RED_THREADS, 0, st>>>(out.v, out.norm, a, x.v, x.norm, b, y.v, y.norm, L5, Vh, partial)
+    if (hasy && norm) AX(true, true);
+    else if (hasy) AX(true, false);
+    else if (norm) AX(false, true);
+    else AX(false, false);
+#undef AX
+    if (norm) final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, nb, result);
+    return (int)cudaGetLastError();
+}
+
+template <class PO, class PX>
+static int axpby_y(Prec py, const SpinorBuf &out, double a, const SpinorBuf &x, double b, const SpinorBuf &y, int L5,
+                   int Vh, double *partial, double *result, cudaStream_t st)
+{
+    switch (py) {
+    case PREC_D: return axpby_xy<PO, PX, PD>(out, a, x, b, y, L5, Vh, partial, result, st);
+    case PREC_S: return axpby_xy<PO, PX, PS>(out, a, x, b, y, L5, Vh, partial, result, st);
+    default: return axpby_xy<PO, PX, PH>(out, a, x, b, y, L5, Vh, partial, result, st);
+    }
+}
+template <class PO>
+static int axpby_x(Prec px, Prec py, const SpinorBuf &out, double a, const SpinorBuf &x, double b, const SpinorBuf &y,
+                   int L5, int Vh, double *partial, double *result, cudaStream_t st)
+{
+    switch (px) {
+    case PREC_D: return axpby_y<PO, PD>(py, out, a, x, b, y, L5, Vh, partial, result, st);
+    case PREC_S: return axpby_y<PO, PS>(py, out, a, x, b, y, L5, Vh, partial, result, st);
+    default: return axpby_y<PO, PH>(py, out, a, x, b, y, L5, Vh, partial, result, st);
+    }
+}
+
+int mdwf_launch_axpby(Prec po, const SpinorBuf &out, double a, Prec px, const SpinorBuf &x, double b, Prec py,
+                      const SpinorBuf &y, int L5, int Vh, double *partial, double *result_dev, cudaStream_t st)
+{
+    switch (po) {
+    case PREC_D: return axpby_x<PD>(px, py, out, a, x, b, y, L5, Vh, partial, result_dev, st);
+    case PREC_S: return axpby_x<PS>(px, py, out, a, x, b, y, L5, Vh, partial, result_dev, st);
+    default: return axpby_x<PH>(px, py, out, a, x, b, y, L5, Vh, partial, result_dev, st);
+    }
+}
+
+template <class PX, class PY>
+static int reduce_xy(int kind, const SpinorBuf &x, const SpinorBuf &y, int L5, int Vh, double *partial,
+                     double *result, cudaStream_t st)
+{
+    const int nb = red_blocks((long long)L5 * Vh);
+    if (kind == 0)
+        reduce_kernel<PX, PY, 0><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, y.v, y.norm, L5, Vh, partial);
+    else
+        reduce_kernel<PX, PY, 1><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, y.v, y.norm, L5, Vh, partial);
+    final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, nb, result);
+    return (int)cudaGetLastError();
+}
+template <class PX>
+static int reduce_y(int kind, Prec py, const SpinorBuf &x, const SpinorBuf &y, int L5, int Vh, double *partial,
+                    double *result, cudaStream_t st)
+{
+    switch (py) {
+    case PREC_D: return reduce_xy<PX, PD>(kind, x, y, L5, Vh, partial, result, st);
+    case PREC_S: return reduce_xy<PX, PS>(kind, x, y, L5, Vh, partial, result, st);
+    default: return reduce_xy<PX, PH>(kind, x, y, L5, Vh, partial, result, st);
+    }
+}
+int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const SpinorBuf &y, int L5, int Vh,
+                       double *partial, double *result_dev, cudaStream_t st)
+{
+    switch (px) {
+    case PREC_D: return reduce_y<PD>(kind, py, x, y, L5, Vh, partial, result_dev, st);
+    case PREC_S: return reduce_y<PS>(kind, py, x, y, L5, Vh, partial, result_dev, st);
+    default: return reduce_y<PH>(kind, py, x, y, L5, Vh, partial, result_dev, st);
+    }
+}
+
+// ---- flat arrays (mdwf_blas_* entry points) -----------------------------------------------------
+template <class T, int KIND>
+__global__ void __launch_bounds__(RED_THREADS) flat_reduce_kernel(const T *x, const T *y, long long n, double *partial)
+{
+    double sum = 0.0;
+    for (long long i = (long long)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (long long)gridDim.x * RED_THREADS) {
+        const double a = (double)x[i];
+        sum += (KIND == 0) ? a * a : a * (double)y[i];
+    }
+    block_partial(sum, partial);
+}
+template <class T>
+__global__ void flat_axpy_kernel(double a, const T *x, T *y, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        y[i] = (T)((double)y[i] + a * (double)x[i]);
+}
+
+int mdwf_launch_flat_reduce(int kind, const void *x, const void *y, long long n, int real_bytes, double *partial,
+                            double *result_dev, cudaStream_t st)
+{
+    const int nb = red_blocks(n / 4 + 1);
+    if (real_bytes == 8) {
+        if (kind == 0) flat_reduce_kernel<double, 0><<<nb, RED_THREADS, 0, st>>>((const double *)x, (const double *)y, n, partial);
+        else flat_reduce_kernel<double, 1><<<nb, RED_THREADS, 0, st>>>((const double *)x, (const double *)y, n, partial);
+    } else {
+        if (kind == 0) flat_reduce_kernel<float, 0><<<nb, RED_THREADS, 0, st>>>((const float *)x, (const float *)y, n, partial);
+        else flat_reduce_kernel<float, 1><<<nb, RED_THREADS, 0, st>>>((const float *)x, (const float *)y, n, partial);
+    }
+    final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, nb, result_dev);
+    return (int)cudaGetLastError();
+}
+int mdwf_launch_flat_axpy(double a, const void *x, void *y, long long n, int real_bytes, cudaStream_t st)
+{
+    const int nb = red_blocks(n / 4 + 1);
+    if (real_bytes == 8) flat_axpy_kernel<double><<<nb, 256, 0, st>>>(a, (const double *)x, (double *)y, n);
+    else flat_axpy_kernel<float><<<nb, 256, 0, st>>>(a, (const float *)x, (float *)y, n);
+    return (int)cudaGetLastError();
+}

@@ -1,0 +1,204 @@
+// layout_kernels.cu -- S0: canonical interchange layouts (include/mdwf.h) <-> even-odd device layouts.
+// One thread per (s, checkerboard site).  Runs once per load / apply / solve, not on the CG hot loop.
+#include "mdwf_device.cuh"
+#include "mdwf_internal.h"
+
+size_t mdwf_spinor_bytes(Prec p, int L5, int Vh)
+{
+    const size_t n = (size_t)L5 * Vh * 24;
+    return p == PREC_D ? n * 8 : (p == PREC_S ? n * 4 : n * 2);
+}
+size_t mdwf_gauge_bytes(Prec p, int Vh, int recon)
+{
+    const size_t n = (size_t)4 * Vh * recon;
+    return p == PREC_D ? n * 8 : (p == PREC_S ? n * 4 : n * 2);
+}
+
+// lexicographic 4D index of checkerboard site cb of the given parity
+__device__ __forceinline__ long cb_to_lex(long cb, int parity, int Lx, int Ly, int Lz)
+{
+    const int Lxh = Lx >> 1;
+    long r = cb;
+    const int xh = (int)(r % Lxh); r /= Lxh;
+    const int y = (int)(r % Ly);   r /= Ly;
+    const int z = (int)(r % Lz);
+    const int t = (int)(r / Lz);
+    const int x = 2 * xh + ((parity + y + z + t) & 1);
+    return x + (long)Lx * (y + (long)Ly * (z + (long)Lz * t));
+}
+
+// canonical site block of 24 reals at element offset `off` (in units of sites) -> device layout
+template <class P, class T>
+__global__ void spinor_in_kernel(const T *canon, void *dst, float *dst_norm, int L5, long Vh, int full, int parity,
+                                 int Lx, int Ly, int Lz, long V4)
+{
+    using R = typename P::R;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)L5 * Vh) return;
+    const int s = (int)(idx / Vh);
+    const long cb = idx - (long)s * Vh;
+    const long site = full ? ((long)s * V4 + cb_to_lex(cb, parity, Lx, Ly, Lz)) : idx;
+    const T *p = canon + site * 24;
+    R v[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) v[k] = (R)p[k];
+    store_spinor<P>(dst, dst_norm, s, cb, Vh, v);
+}
+template <class P, class T>
+__global__ void spinor_out_kernel(const void *src, const float *src_norm, T *canon, int L5, long Vh, int full,
+                                  int parity, int Lx, int Ly, int Lz, long V4)
+{
+    using R = typename P::R;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)L5 * Vh) return;
+    const int s = (int)(idx / Vh);
+    const long cb = idx - (long)s * Vh;
+    const long site = full ? ((long)s * V4 + cb_to_lex(cb, parity, Lx, Ly, Lz)) : idx;
+    T *p = canon + site * 24;
+    R v[24];
+    load_spinor<P>(src, src_norm, s, cb, Vh, v);
+#pragma unroll
+    for (int k = 0; k < 24; k++) p[k] = (T)v[k];
+}
+
+MDWF_DEV double2 gpack(double re, double im, double2 *) { return make_double2(re, im); }
+MDWF_DEV float2 gpack(double re, double im, float2 *) { return make_float2((float)re, (float)im); }
+MDWF_DEV short2 gpack(double re, double im, short2 *)
+{
+    return make_short2((short)__double2int_rn(re * (double)MDWF_FIXED_MAX), (short)__double2int_rn(im * (double)MDWF_FIXED_MAX));
+}
+
+template <class P, class T>
+__global__ void gauge_in_kernel(const T *canon, void *dst, long Vh, int parity, int recon, int Lx, int Ly, int Lz)
+{
+    using G = typename P::G;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 4 * Vh) return;
+    const int mu = (int)(idx / Vh);
+    const long cb = idx - (long)mu * Vh;
+    const long lex = cb_to_lex(cb, parity, Lx, Ly, Lz);
+    const T *p = canon + (lex * 4 + mu) * 18;
+    const int NK = recon >> 1;
+    G *q = reinterpret_cast<G *>(dst) + ((long)mu * NK) * Vh + cb;
+    for (int k = 0; k < NK; k++) q[(long)k * Vh] = gpack((double)p[2 * k], (double)p[2 * k + 1], (G *)nullptr);
+}
+
+template <class P>
+static int spinor_in(const void *canon, int real_bytes, const SpinorBuf &dst, int L5, long Vh, int full, int parity,
+                     const int *L, cudaStream_t st)
+{
+    const long n = (long)L5 * Vh;
+    const int T = 128;
+    const unsigned nb = (unsigned)((n + T - 1) / T);
+    const int Lx = L ? L[0] : 2, Ly = L ? L[1] : 1, Lz = L ? L[2] : 1;
+    const long V4 = 2 * Vh;
+    if (real_bytes == 8)
+        spinor_in_kernel<P, double><<<nb, T, 0, st>>>((const double *)canon, dst.v, dst.norm, L5, Vh, full, parity, Lx, Ly, Lz, V4);
+    else
+        spinor_in_kernel<P, float><<<nb, T, 0, st>>>((const float *)canon, dst.v, dst.norm, L5, Vh, full, parity, Lx, Ly, Lz, V4);
+    return (int)cudaGetLastError();
+}
+template <class P>
+static int spinor_out(const SpinorBuf &src, void *canon, int real_bytes, int L5, long Vh, int full, int parity,
+                      const int *L, cudaStream_t st)
+{
+    const long n = (long)L5 * Vh;
+    const int T = 128;
+    const unsigned nb = (unsigned)((n + T - 1) / T);
+    const int Lx = L ? L[0] : 2, Ly = L ? L[1] : 1, Lz = L ? L[2] : 1;
+    const long V4 = 2 * Vh;
+    if (real_bytes == 8)
+        spinor_out_kernel<P, double><<<nb, T, 0, st>>>(src.v, src.norm, (double *)canon, L5, Vh, full, parity, Lx, Ly, Lz, V4);
+    else
+        spinor_out_kernel<P, float><<<nb, T, 0, st>>>(src.v, src.norm, (float *)canon, L5, Vh, full, parity, Lx, Ly, Lz, V4);
+    return (int)cudaGetLastError();
+}
+
+#define DISPATCH_P(p, CALL)                      \
+    switch (p) {                                 \
+    case PREC_D: return CALL(PD);                \
+    case PREC_S: return CALL(PS);                \
+    default: return CALL(PH);                    \
+    }
+
+int mdwf_launch_parity_in(Prec p, const void *canon, int real_bytes, const SpinorBuf &dst, int L5, int Vh,
+                          cudaStream_t st)
+{
+#define C(PP) spinor_in<PP>(canon, real_bytes, dst, L5, Vh, 0, 0, nullptr, st)
+    DISPATCH_P(p, C)
+#undef C
+}
+int mdwf_launch_parity_out(Prec p, const SpinorBuf &src, void *canon, int real_bytes, int L5, int Vh,
+                           cudaStream_t st)
+{
+#define C(PP) spinor_out<PP>(src, canon, real_bytes, L5, Vh, 0, 0, nullptr, st)
+    DISPATCH_P(p, C)
+#undef C
+}
+int mdwf_launch_full_in(Prec p, const void *canon, int real_bytes, const SpinorBuf &dst, const int *L, int L5,
+                        int parity, cudaStream_t st)
+{
+    const long Vh = (long)L[0] * L[1] * L[2] * L[3] / 2;
+#define C(PP) spinor_in<PP>(canon, real_bytes, dst, L5, Vh, 1, parity, L, st)
+    DISPATCH_P(p, C)
+#undef C
+}
+int mdwf_launch_full_out(Prec p, const SpinorBuf &src, void *canon, int real_bytes, const int *L, int L5,
+                         int parity, cudaStream_t st)
+{
+    const long Vh = (long)L[0] * L[1] * L[2] * L[3] / 2;
+#define C(PP) spinor_out<PP>(src, canon, real_bytes, L5, Vh, 1, parity, L, st)
+    DISPATCH_P(p, C)
+#undef C
+}
+
+template <class P>
+static int gauge_in(const void *canon, int real_bytes, void *dst, const int *L, int parity, int recon, cudaStream_t st)
+{
+    const long Vh = (long)L[0] * L[1] * L[2] * L[3] / 2;
+    const int T = 128;
+    const unsigned nb = (unsigned)((4 * Vh + T - 1) / T);
+    if (real_bytes == 8)
+        gauge_in_kernel<P, double><<<nb, T, 0, st>>>((const double *)canon, dst, Vh, parity, recon, L[0], L[1], L[2]);
+    else
+        gauge_in_kernel<P, float><<<nb, T, 0, st>>>((const float *)canon, dst, Vh, parity, recon, L[0], L[1], L[2]);
+    return (int)cudaGetLastError();
+}
+int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, const int *L, int parity, int recon,
+                         cudaStream_t st)
+{
+#define C(PP) gauge_in<PP>(canon, real_bytes, dst, L, parity, recon, st)
+    DISPATCH_P(p, C)
+#undef C
+}
+
+// ---- timing inputs: hash-filled vectors ------------------------------------------------------------
+template <class P>
+__global__ void fill_kernel(void *dst, float *dst_norm, int L5, long Vh, unsigned seed)
+{
+    using R = typename P::R;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)L5 * Vh) return;
+    const int s = (int)(idx / Vh);
+    const long cb = idx - (long)s * Vh;
+    R v[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) {
+        unsigned h = (unsigned)(idx * 24 + k) * 2654435761u + seed;
+        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13; h *= 3266489917u; h ^= h >> 16;
+        v[k] = (R)((double)h * (2.0 / 4294967295.0) - 1.0);
+    }
+    store_spinor<P>(dst, dst_norm, s, cb, Vh, v);
+}
+int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st)
+{
+    const long n = (long)L5 * Vh;
+    const int T = 128;
+    const unsigned nb = (unsigned)((n + T - 1) / T);
+    switch (p) {
+    case PREC_D: fill_kernel<PD><<<nb, T, 0, st>>>(dst.v, dst.norm, L5, Vh, seed); break;
+    case PREC_S: fill_kernel<PS><<<nb, T, 0, st>>>(dst.v, dst.norm, L5, Vh, seed); break;
+    default: fill_kernel<PH><<<nb, T, 0, st>>>(dst.v, dst.norm, L5, Vh, seed); break;
+    }
+    return (int)cudaGetLastError();
+}

@@ -1,0 +1,715 @@
+// mdwf_api.cu -- the C ABI of include/mdwf.h: context, options, gauge load, operator application,
+// mixed-precision CG with reliable updates (S8-S10).  Host logic only; every arithmetic step runs in
+// the kernels of hop_kernels.cuh / blas_kernels.cu / layout_kernels.cu.
+#include "../../include/mdwf.h"
+#include "mdwf_internal.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+int mdwf_launch_hop_D(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop_S(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
+int mdwf_launch_sdense_S(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
+int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
+
+int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
+{
+    switch (p) {
+    case PREC_D: return mdwf_launch_hop_D(dag, pre, post, own, a, st);
+    case PREC_S: return mdwf_launch_hop_S(dag, pre, post, own, a, st);
+    default: return mdwf_launch_hop_H(dag, pre, post, own, a, st);
+    }
+}
+int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, const void *dense,
+                       cudaStream_t st)
+{
+    switch (p) {
+    case PREC_D: return mdwf_launch_sdense_D(L5, Vh, in, out, dense, st);
+    case PREC_S: return mdwf_launch_sdense_S(L5, Vh, in, out, dense, st);
+    default: return mdwf_launch_sdense_H(L5, Vh, in, out, dense, st);
+    }
+}
+
+enum { DENSE_BAINV = 0, DENSE_BAINV_DAG = 1, DENSE_AINV = 2, DENSE_KINDS = 3 };
+
+struct mdwf_ctx {
+    int L[4];
+    int L5;
+    int Vh;
+    double M5, b5, c5, mf, alpha, beta;
+    cudaStream_t st = 0;
+    int recon_opt = 18, recon = 18;
+    int ladder = 0;          // 0 d, 1 ds, 2 dh, 3 dsh
+    int apply_prec = -1;     // -1 auto
+    double delta = 0.1;
+    int max_update_interval = 0;
+    bool gauge_loaded = false;
+    void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
+    void *dense[2][DENSE_KINDS] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [0] double, [1] float
+    std::map<std::string, SpinorBuf> pool;
+    std::map<std::string, void *> raw;
+    double *partial = nullptr, *result_dev = nullptr, *result_host = nullptr;
+    // stats
+    double launches = 0, iterations = 0, reliable_updates = 0, solve_seconds = 0, true_residual = 0;
+    double op_applications = 0, sloppy_applications = 0;
+    std::string err;
+};
+
+#define CUDA_OK(ctx, call)                                                                          \
+    do {                                                                                            \
+        cudaError_t e_ = (cudaError_t)(call);                                                       \
+        if (e_ != cudaSuccess) {                                                                    \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                        \
+            return (e_ == cudaErrorMemoryAllocation) ? MDWF_ENOMEM : MDWF_ECUDA;                    \
+        }                                                                                           \
+    } while (0)
+#define TRY(call)                \
+    do {                         \
+        int rc_ = (call);        \
+        if (rc_ != MDWF_OK) return rc_; \
+    } while (0)
+
+// ---- fifth-dimension tables (host, fp64; independent numeric inverse, not a closed form) ---------
+static void invert(std::vector<double> &a, int n)   // Gauss-Jordan with partial pivoting, in place
+{
+    std::vector<double> inv(n * n, 0.0);
+    for (int i = 0; i < n; i++) inv[i * n + i] = 1.0;
+    for (int c = 0; c < n; c++) {
+        int piv = c;
+        for (int r = c + 1; r < n; r++)
+            if (std::fabs(a[r * n + c]) > std::fabs(a[piv * n + c])) piv = r;
+        for (int k = 0; k < n; k++) { std::swap(a[c * n + k], a[piv * n + k]); std::swap(inv[c * n + k], inv[piv * n + k]); }
+        const double d = 1.0 / a[c * n + c];
+        for (int k = 0; k < n; k++) { a[c * n + k] *= d; inv[c * n + k] *= d; }
+        for (int r = 0; r < n; r++)
+            if (r != c) {
+                const double f = a[r * n + c];
+                if (f != 0.0)
+                    for (int k = 0; k < n; k++) { a[r * n + k] -= f * a[c * n + k]; inv[r * n + k] -= f * inv[c * n + k]; }
+            }
+    }
+    a = inv;
+}
+
+static void build_tables(const mdwf_ctx *c, std::vector<double> out[DENSE_KINDS])
+{
+    const int n = c->L5;
+    // shift matrix T: (T v)_s = v_{s-1}, wall factor -m_f at the wrap.  P+ block of Lambda is T, P- block T^T.
+    std::vector<double> T(n * n, 0.0);
+    for (int s = 1; s < n; s++) T[s * n + s - 1] = 1.0;
+    T[0 * n + n - 1] += -c->mf;
+    std::vector<double> Ap(n * n), Am(n * n), Bp(n * n), Bm(n * n);
+    for (int i = 0; i < n; i++)
+        for (int j = 0; j < n; j++) {
+            const double id = (i == j) ? 1.0 : 0.0;
+            Ap[i * n + j] = c->alpha * id + c->beta * T[i * n + j];
+            Am[i * n + j] = c->alpha * id + c->beta * T[j * n + i];
+            Bp[i * n + j] = c->b5 * id + c->c5 * T[i * n + j];
+            Bm[i * n + j] = c->b5 * id + c->c5 * T[j * n + i];
+        }
+    std::vector<double> Aip = Ap, Aim = Am;
+    invert(Aip, n);
+    invert(Aim, n);
+    for (int k = 0; k < DENSE_KINDS; k++) out[k].assign(2 * n * n, 0.0);
+    for (int i = 0; i < n; i++)
+        for (int j = 0; j < n; j++) {
+            double sp = 0, sm = 0;
+            for (int k = 0; k < n; k++) { sp += Bp[i * n + k] * Aip[k * n + j]; sm += Bm[i * n + k] * Aim[k * n + j]; }
+            out[DENSE_BAINV][i * n + j] = sp;
+            out[DENSE_BAINV][n * n + i * n + j] = sm;
+            out[DENSE_BAINV_DAG][j * n + i] = sp;            // (B A^{-1})^T per chirality = A^{-+} B^+
+            out[DENSE_BAINV_DAG][n * n + j * n + i] = sm;
+            out[DENSE_AINV][i * n + j] = Aip[i * n + j];
+            out[DENSE_AINV][n * n + i * n + j] = Aim[i * n + j];
+        }
+}
+
+// ---- memory helpers ----------------------------------------------------------------------------
+static int get_spinor(mdwf_ctx *c, const std::string &name, Prec p, SpinorBuf *out)
+{
+    const std::string key = name + (p == PREC_D ? ".d" : p == PREC_S ? ".s" : ".h");
+    auto it = c->pool.find(key);
+    if (it != c->pool.end()) { *out = it->second; return MDWF_OK; }
+    SpinorBuf b;
+    CUDA_OK(c, cudaMalloc(&b.v, mdwf_spinor_bytes(p, c->L5, c->Vh)));
+    if (p == PREC_H) CUDA_OK(c, cudaMalloc((void **)&b.norm, sizeof(float) * (size_t)c->L5 * c->Vh));
+    c->pool[key] = b;
+    *out = b;
+    return MDWF_OK;
+}
+static int get_raw(mdwf_ctx *c, const std::string &name, size_t bytes, void **out)
+{
+    auto it = c->raw.find(name);
+    if (it != c->raw.end()) { *out = it->second; return MDWF_OK; }
+    void *p = nullptr;
+    CUDA_OK(c, cudaMalloc(&p, bytes));
+    c->raw[name] = p;
+    *out = p;
+    return MDWF_OK;
+}
+static void free_pool(mdwf_ctx *c)
+{
+    for (auto &kv : c->pool) { cudaFree(kv.second.v); if (kv.second.norm) cudaFree(kv.second.norm); }
+    c->pool.clear();
+    for (auto &kv : c->raw) cudaFree(kv.second);
+    c->raw.clear();
+}
+
+static int ensure_scalars(mdwf_ctx *c)
+{
+    if (c->partial) return MDWF_OK;
+    CUDA_OK(c, cudaMalloc((void **)&c->partial, sizeof(double) * mdwf_reduce_max_blocks()));
+    CUDA_OK(c, cudaMalloc((void **)&c->result_dev, sizeof(double) * 4));
+    CUDA_OK(c, cudaMallocHost((void **)&c->result_host, sizeof(double) * 4));
+    return MDWF_OK;
+}
+static int fetch_scalar(mdwf_ctx *c, double *out)
+{
+    CUDA_OK(c, cudaMemcpyAsync(c->result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    *out = c->result_host[0];
+    return MDWF_OK;
+}
+
+// ---- BLAS-1 wrappers (count launches) ------------------------------------------------------------
+static int v_axpby(mdwf_ctx *c, Prec po, const SpinorBuf &out, double a, Prec px, const SpinorBuf &x, double b, Prec py,
+                   const SpinorBuf *y, double *norm2_out)
+{
+    SpinorBuf none;
+    TRY(ensure_scalars(c));
+    CUDA_OK(c, mdwf_launch_axpby(po, out, a, px, x, b, py, y ? *y : none, c->L5, c->Vh, norm2_out ? c->partial : nullptr,
+                                 c->result_dev, c->st));
+    c->launches += norm2_out ? 2 : 1;
+    if (norm2_out) TRY(fetch_scalar(c, norm2_out));
+    return MDWF_OK;
+}
+static int v_norm2(mdwf_ctx *c, Prec p, const SpinorBuf &x, double *out)
+{
+    TRY(ensure_scalars(c));
+    CUDA_OK(c, mdwf_launch_reduce(0, p, x, p, x, c->L5, c->Vh, c->partial, c->result_dev, c->st));
+    c->launches += 2;
+    return fetch_scalar(c, out);
+}
+static int v_zero(mdwf_ctx *c, Prec p, const SpinorBuf &x)
+{
+    CUDA_OK(c, cudaMemsetAsync(x.v, 0, mdwf_spinor_bytes(p, c->L5, c->Vh), c->st));
+    if (p == PREC_H) CUDA_OK(c, cudaMemsetAsync(x.norm, 0, sizeof(float) * (size_t)c->L5 * c->Vh, c->st));
+    return MDWF_OK;
+}
+
+// ---- operator building blocks ---------------------------------------------------------------------
+static const void *dense_ptr(const mdwf_ctx *c, Prec p, int kind) { return c->dense[p == PREC_D ? 0 : 1][kind]; }
+
+static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const SpinorBuf &in, const SpinorBuf *own,
+                         const SpinorBuf &out)
+{
+    HopArgs a;
+    memset(&a, 0, sizeof(a));
+    for (int d = 0; d < 4; d++) a.L[d] = c->L[d];
+    a.L5 = c->L5;
+    a.Vh = c->Vh;
+    a.parity_out = parity_out;
+    a.in = in.v; a.in_norm = in.norm;
+    a.own = own ? own->v : nullptr; a.own_norm = own ? own->norm : nullptr;
+    a.out = out.v; a.out_norm = out.norm;
+    a.gauge_same = c->gauge[p][parity_out];
+    a.gauge_other = c->gauge[p][1 - parity_out];
+    a.recon = c->recon;
+    a.mf = c->mf;
+    return a;
+}
+static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, const HopArgs &a)
+{
+    CUDA_OK(c, mdwf_launch_hop(p, dag, pre, post, own, a, c->st));
+    c->launches += 1;
+    return MDWF_OK;
+}
+
+// Mpc in_o = A in_o - (1/4) H_oe [B A^{-1}] H_eo [B in_o];  tmp holds the even-site intermediate.
+static int op_Mpc_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp)
+{
+    HopArgs k1 = base_args(c, p, 0, in, nullptr, tmp);        // K1: t_e = (B A^{-1}) H_eo (B in_o)
+    k1.coef_hop = 1.0; k1.pre_d = c->b5; k1.pre_o = c->c5; k1.dense = dense_ptr(c, p, DENSE_BAINV);
+    return run_hop(c, p, 0, 1, 1, 0, k1);
+}
+static int op_Mpc_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2: out_o = A in_o - (1/4) H_oe t_e
+    k2.coef_hop = -0.25; k2.own_d = c->alpha; k2.own_o = c->beta;
+    return run_hop(c, p, 0, 0, 0, 2, k2);
+}
+static int op_Mpc(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    TRY(op_Mpc_k1(c, p, in, tmp));
+    TRY(op_Mpc_k2(c, p, in, tmp, out));
+    c->op_applications += 1;
+    if (p != PREC_D) c->sloppy_applications += 1;
+    return MDWF_OK;
+}
+// Mpc^+ in_o = A^+ in_o - (1/4) B^+ H'_oe [A^{-+} B^+] H'_eo in_o
+static int op_Mpcdag_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp)
+{
+    HopArgs k1 = base_args(c, p, 0, in, nullptr, tmp);        // K1+: u_e = (A^{-+} B^+) H'_eo in_o
+    k1.coef_hop = 1.0; k1.dense = dense_ptr(c, p, DENSE_BAINV_DAG);
+    return run_hop(c, p, 1, 0, 1, 0, k1);
+}
+static int op_Mpcdag_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2+: out_o = A^+ in_o - (1/4) B^+ H'_oe u_e
+    k2.coef_hop = -0.25; k2.post_d = c->b5; k2.post_o = c->c5; k2.own_d = c->alpha; k2.own_o = c->beta;
+    return run_hop(c, p, 1, 0, 2, 3, k2);
+}
+static int op_Mpcdag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    TRY(op_Mpcdag_k1(c, p, in, tmp));
+    TRY(op_Mpcdag_k2(c, p, in, tmp, out));
+    c->op_applications += 1;
+    if (p != PREC_D) c->sloppy_applications += 1;
+    return MDWF_OK;
+}
+// one parity of D: out_p = A in_p - (1/2) H_{p,pbar} B in_pbar
+static int op_D_parity(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_other, const SpinorBuf &in_same,
+                       const SpinorBuf &out)
+{
+    HopArgs a = base_args(c, p, parity, in_other, &in_same, out);
+    a.coef_hop = -0.5; a.pre_d = c->b5; a.pre_o = c->c5; a.own_d = c->alpha; a.own_o = c->beta;
+    return run_hop(c, p, 0, 1, 0, 2, a);
+}
+// one parity of D^+: out_p = A^+ in_p - (1/2) B^+ H'_{p,pbar} in_pbar
+static int op_Ddag_parity(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_other, const SpinorBuf &in_same,
+                          const SpinorBuf &out)
+{
+    HopArgs a = base_args(c, p, parity, in_other, &in_same, out);
+    a.coef_hop = -0.5; a.post_d = c->b5; a.post_o = c->c5; a.own_d = c->alpha; a.own_o = c->beta;
+    return run_hop(c, p, 1, 0, 2, 3, a);
+}
+// out_p = own_p + (1/2) H_{p,pbar} B in_pbar   ( = own_p - D_{p,pbar} in_pbar ), Schur preparation / reconstruction
+static int op_schur_hop(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_other, const SpinorBuf &own,
+                        const SpinorBuf &out)
+{
+    HopArgs a = base_args(c, p, parity, in_other, &own, out);
+    a.coef_hop = 0.5; a.pre_d = c->b5; a.pre_o = c->c5;
+    return run_hop(c, p, 0, 1, 0, 1, a);
+}
+static int op_Ainv(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out)
+{
+    CUDA_OK(c, mdwf_launch_sdense(p, c->L5, c->Vh, in, out, dense_ptr(c, p, DENSE_AINV), c->st));
+    c->launches += 1;
+    return MDWF_OK;
+}
+
+static int check_ready(mdwf_ctx *c)
+{
+    if (!c) return MDWF_EARG;
+    if (!c->gauge_loaded) { c->err = "gauge field not loaded"; return MDWF_ENOGAUGE; }
+    return MDWF_OK;
+}
+
+// =====================================================================================================
+extern "C" {
+
+int mdwf_create(mdwf_ctx **out, int Lx, int Ly, int Lz, int Lt, int L5, double M5, double b5, double c5, double m_f)
+{
+    if (!out) return MDWF_EARG;
+    *out = nullptr;
+    const int L[4] = {Lx, Ly, Lz, Lt};
+    for (int d = 0; d < 4; d++)
+        if (L[d] < 2 || (L[d] & 1)) return MDWF_EARG;
+    if (L5 < 2 || L5 > 32) return MDWF_EARG;
+    const long long V4 = (long long)Lx * Ly * Lz * Lt;
+    if (V4 / 2 > 0x7fffffffLL / 32) return MDWF_EARG;     // L5 * Vh must fit comfortably in int
+    mdwf_ctx *c = new mdwf_ctx();
+    for (int d = 0; d < 4; d++) c->L[d] = L[d];
+    c->L5 = L5;
+    c->Vh = (int)(V4 / 2);
+    c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = m_f;
+    c->alpha = b5 * (4.0 - M5) + 1.0;
+    c->beta = c5 * (4.0 - M5) - 1.0;
+    if (c->alpha == 0.0) { delete c; return MDWF_EARG; }
+    *out = c;
+    return MDWF_OK;
+}
+
+int mdwf_destroy(mdwf_ctx *c)
+{
+    if (!c) return MDWF_EARG;
+    free_pool(c);
+    for (int p = 0; p < 3; p++)
+        for (int q = 0; q < 2; q++)
+            if (c->gauge[p][q]) cudaFree(c->gauge[p][q]);
+    for (int p = 0; p < 2; p++)
+        for (int k = 0; k < DENSE_KINDS; k++)
+            if (c->dense[p][k]) cudaFree(c->dense[p][k]);
+    if (c->partial) cudaFree(c->partial);
+    if (c->result_dev) cudaFree(c->result_dev);
+    if (c->result_host) cudaFreeHost(c->result_host);
+    delete c;
+    return MDWF_OK;
+}
+
+const char *mdwf_last_error(const mdwf_ctx *c) { return c ? c->err.c_str() : "null context"; }
+int mdwf_flops_per_site(const mdwf_ctx *c) { return c ? 2880 + 48 * c->L5 : MDWF_EARG; }
+
+int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
+{
+    if (!c || !key || !value) return MDWF_EARG;
+    const std::string k(key), v(value);
+    if (k == "ladder") {
+        if (v == "d") c->ladder = 0;
+        else if (v == "ds") c->ladder = 1;
+        else if (v == "dh") c->ladder = 2;
+        else if (v == "dsh") c->ladder = 3;
+        else { c->err = "ladder must be d|ds|dh|dsh"; return MDWF_EARG; }
+    } else if (k == "apply_precision") {
+        if (v == "auto") c->apply_prec = -1;
+        else if (v == "fp64") c->apply_prec = PREC_D;
+        else if (v == "fp32") c->apply_prec = PREC_S;
+        else if (v == "half") c->apply_prec = PREC_H;
+        else { c->err = "apply_precision must be auto|fp64|fp32|half"; return MDWF_EARG; }
+    } else if (k == "reconstruct") {
+        if (v == "18") c->recon_opt = 18;
+        else if (v == "12") c->recon_opt = 12;
+        else { c->err = "reconstruct must be 18|12"; return MDWF_EARG; }
+    } else if (k == "reliable_delta") {
+        const double d = atof(value);
+        if (!(d > 0.0 && d < 1.0)) { c->err = "reliable_delta must be in (0,1)"; return MDWF_EARG; }
+        c->delta = d;
+    } else if (k == "max_update_interval") {
+        c->max_update_interval = atoi(value);
+    } else if (k == "stream") {
+        c->st = (cudaStream_t)(uintptr_t)strtoull(value, nullptr, 10);
+    } else if (k == "matpc") {
+        if (v != "asym") { c->err = "only matpc=asym is implemented"; return MDWF_EARG; }
+    } else {
+        c->err = "unknown option " + k;
+        return MDWF_EARG;
+    }
+    return MDWF_OK;
+}
+
+int mdwf_load_gauge(mdwf_ctx *c, const void *U_dev, int real_bytes)
+{
+    if (!c || !U_dev || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    int ndev = 0;
+    CUDA_OK(c, cudaGetDeviceCount(&ndev));
+    const int recon = c->recon_opt;
+    if (c->gauge_loaded && recon != c->recon) {
+        for (int p = 0; p < 3; p++)
+            for (int q = 0; q < 2; q++) { cudaFree(c->gauge[p][q]); c->gauge[p][q] = nullptr; }
+    }
+    for (int p = 0; p < 3; p++)
+        for (int q = 0; q < 2; q++) {
+            if (!c->gauge[p][q]) CUDA_OK(c, cudaMalloc(&c->gauge[p][q], mdwf_gauge_bytes((Prec)p, c->Vh, recon)));
+            CUDA_OK(c, mdwf_launch_gauge_in((Prec)p, U_dev, real_bytes, c->gauge[p][q], c->L, q, recon, c->st));
+            c->launches += 1;
+        }
+    c->recon = recon;
+    // fifth-dimension tables in fp64 and fp32
+    std::vector<double> tab[DENSE_KINDS];
+    build_tables(c, tab);
+    for (int k = 0; k < DENSE_KINDS; k++) {
+        const size_t n = tab[k].size();
+        std::vector<float> tf(n);
+        for (size_t i = 0; i < n; i++) tf[i] = (float)tab[k][i];
+        if (!c->dense[0][k]) CUDA_OK(c, cudaMalloc(&c->dense[0][k], n * sizeof(double)));
+        if (!c->dense[1][k]) CUDA_OK(c, cudaMalloc(&c->dense[1][k], n * sizeof(float)));
+        CUDA_OK(c, cudaMemcpy(c->dense[0][k], tab[k].data(), n * sizeof(double), cudaMemcpyHostToDevice));
+        CUDA_OK(c, cudaMemcpy(c->dense[1][k], tf.data(), n * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    c->gauge_loaded = true;
+    return MDWF_OK;
+}
+
+int mdwf_load_gauge_host(mdwf_ctx *c, const void *U_host, int real_bytes)
+{
+    if (!c || !U_host || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    const size_t bytes = (size_t)2 * c->Vh * 4 * 18 * real_bytes;
+    void *tmp = nullptr;
+    CUDA_OK(c, cudaMalloc(&tmp, bytes));
+    cudaError_t e = cudaMemcpy(tmp, U_host, bytes, cudaMemcpyHostToDevice);
+    int rc = MDWF_OK;
+    if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = MDWF_ECUDA; }
+    else rc = mdwf_load_gauge(c, tmp, real_bytes);
+    cudaFree(tmp);
+    return rc;
+}
+
+int mdwf_apply(mdwf_ctx *c, int op, const void *in_dev, void *out_dev, int real_bytes)
+{
+    TRY(check_ready(c));
+    if (!in_dev || !out_dev || in_dev == out_dev || (real_bytes != 8 && real_bytes != 4) || op < 0 || op > 4) {
+        c->err = "mdwf_apply: bad argument";
+        return MDWF_EARG;
+    }
+    const Prec p = c->apply_prec >= 0 ? (Prec)c->apply_prec : (real_bytes == 8 ? PREC_D : PREC_S);
+    SpinorBuf a, b, t, u;
+    TRY(get_spinor(c, "ap.a", p, &a));
+    TRY(get_spinor(c, "ap.b", p, &b));
+    TRY(get_spinor(c, "ap.t", p, &t));
+    if (op <= MDWF_OP_MDAGM) {
+        CUDA_OK(c, mdwf_launch_parity_in(p, in_dev, real_bytes, a, c->L5, c->Vh, c->st));
+        if (op == MDWF_OP_MPC) TRY(op_Mpc(c, p, a, t, b));
+        else if (op == MDWF_OP_MPCDAG) TRY(op_Mpcdag(c, p, a, t, b));
+        else {
+            TRY(get_spinor(c, "ap.u", p, &u));
+            TRY(op_Mpc(c, p, a, t, u));
+            TRY(op_Mpcdag(c, p, u, t, b));
+        }
+        CUDA_OK(c, mdwf_launch_parity_out(p, b, out_dev, real_bytes, c->L5, c->Vh, c->st));
+        c->launches += 2;
+    } else {
+        // a = even part, b = odd part of the input; t / u = even / odd part of the output
+        TRY(get_spinor(c, "ap.u", p, &u));
+        CUDA_OK(c, mdwf_launch_full_in(p, in_dev, real_bytes, a, c->L, c->L5, 0, c->st));
+        CUDA_OK(c, mdwf_launch_full_in(p, in_dev, real_bytes, b, c->L, c->L5, 1, c->st));
+        if (op == MDWF_OP_D) {
+            TRY(op_D_parity(c, p, 0, b, a, t));
+            TRY(op_D_parity(c, p, 1, a, b, u));
+        } else {
+            TRY(op_Ddag_parity(c, p, 0, b, a, t));
+            TRY(op_Ddag_parity(c, p, 1, a, b, u));
+        }
+        CUDA_OK(c, mdwf_launch_full_out(p, t, out_dev, real_bytes, c->L, c->L5, 0, c->st));
+        CUDA_OK(c, mdwf_launch_full_out(p, u, out_dev, real_bytes, c->L, c->L5, 1, c->st));
+        c->launches += 4;
+    }
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
+}
+
+// ---- S8-S10: Schur preparation, CG on the normal equations with reliable updates, reconstruction -------
+static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double tol, int maxiter, int *iters_out,
+                        double *true_res_out)
+{
+    const Prec PDd = PREC_D;
+    const Prec ps = (c->ladder == 0) ? PREC_D : (c->ladder == 1 ? PREC_S : PREC_H);   // sloppy operator / Krylov vectors
+    const Prec pxl = (c->ladder == 0) ? PREC_D : (c->ladder == 2 ? PREC_H : PREC_S);  // sloppy solution accumulator
+    SpinorBuf be, bo, bp, xhi, rhi, te;
+    TRY(get_spinor(c, "sv.be", PDd, &be));
+    TRY(get_spinor(c, "sv.bo", PDd, &bo));
+    TRY(get_spinor(c, "sv.bp", PDd, &bp));
+    TRY(get_spinor(c, "sv.xhi", PDd, &xhi));
+    TRY(get_spinor(c, "sv.rhi", PDd, &rhi));
+    TRY(get_spinor(c, "sv.te", PDd, &te));
+    SpinorBuf rs, g, p, q, ts, xlo;
+    TRY(get_spinor(c, "sv.rs", ps, &rs));
+    TRY(get_spinor(c, "sv.g", ps, &g));
+    TRY(get_spinor(c, "sv.p", ps, &p));
+    TRY(get_spinor(c, "sv.q", ps, &q));
+    TRY(get_spinor(c, "sv.ts", ps, &ts));
+    TRY(get_spinor(c, "sv.xlo", pxl, &xlo));
+
+    c->iterations = 0; c->reliable_updates = 0; c->op_applications = 0; c->sloppy_applications = 0;
+
+    // S0: canonical full 5D source -> even / odd device vectors (fp64)
+    CUDA_OK(c, mdwf_launch_full_in(PDd, src_dev, 8, be, c->L, c->L5, 0, c->st));
+    CUDA_OK(c, mdwf_launch_full_in(PDd, src_dev, 8, bo, c->L, c->L5, 1, c->st));
+    c->launches += 2;
+    double be2 = 0, bo2 = 0;
+    TRY(v_norm2(c, PDd, be, &be2));
+    TRY(v_norm2(c, PDd, bo, &bo2));
+    const double bnorm = std::sqrt(be2 + bo2);
+    if (bnorm == 0.0) {
+        CUDA_OK(c, cudaMemsetAsync(sol_dev, 0, (size_t)2 * c->Vh * c->L5 * 24 * 8, c->st));
+        CUDA_OK(c, cudaStreamSynchronize(c->st));
+        if (iters_out) *iters_out = 0;
+        if (true_res_out) *true_res_out = 0.0;
+        return MDWF_OK;
+    }
+    // S10: b'_o = b_o - D_oe A^{-1} b_e
+    TRY(op_Ainv(c, PDd, be, rhi));
+    TRY(op_schur_hop(c, PDd, 1, rhi, bo, bp));
+    // ||b - D x|| = ||b' - Mpc x_o|| once x_e is reconstructed, so the CG target is absolute: tol * ||b||
+    const double target = tol * bnorm;
+
+    TRY(v_zero(c, PDd, xhi));
+    TRY(v_zero(c, pxl, xlo));
+    double r2 = 0;
+    TRY(v_axpby(c, PDd, rhi, 1.0, PDd, bp, 0.0, PDd, nullptr, &r2));        // r_hi = b'
+    double rn = std::sqrt(r2), rmax = rn;
+    bool converged = rn <= target;
+    int k = 0, since_update = 0;
+    if (!converged) {
+        TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr)); // r_s = convert(r_hi)
+        TRY(op_Mpcdag(c, ps, rs, ts, g));                                   // g = Mpc^+ r
+        double gam = 0;
+        TRY(v_axpby(c, ps, p, 1.0, ps, g, 0.0, ps, nullptr, &gam));         // p = g, gam = ||g||^2
+        while (k < maxiter && !converged) {
+            double qq = 0;
+            TRY(op_Mpc(c, ps, p, ts, q));                                   // q = Mpc p
+            TRY(v_norm2(c, ps, q, &qq));
+            if (!(qq > 0.0) || !(gam > 0.0)) break;
+            const double a = gam / qq;
+            TRY(v_axpby(c, pxl, xlo, a, ps, p, 1.0, pxl, &xlo, nullptr));   // x_lo += a p
+            TRY(v_axpby(c, ps, rs, -a, ps, q, 1.0, ps, &rs, &r2));          // r -= a q, ||r||^2
+            k++; since_update++;
+            rn = std::sqrt(r2);
+            const bool update = (rn < c->delta * rmax) || (rn <= target) ||
+                                (c->max_update_interval > 0 && since_update >= c->max_update_interval);
+            if (update) {
+                // reliable update: fold x_lo into x_hi and recompute the true residual in fp64
+                TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
+                TRY(v_zero(c, pxl, xlo));
+                TRY(op_Mpc(c, PDd, xhi, te, rhi));
+                TRY(v_axpby(c, PDd, rhi, 1.0, PDd, bp, -1.0, PDd, &rhi, &r2));   // r_hi = b' - Mpc x_hi
+                rn = std::sqrt(r2);
+                c->reliable_updates += 1;
+                since_update = 0;
+                if (rn <= target) { converged = true; break; }
+                TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr));
+                rmax = rn;
+            }
+            TRY(op_Mpcdag(c, ps, rs, ts, g));                               // g = Mpc^+ r
+            double gam_new = 0;
+            TRY(v_norm2(c, ps, g, &gam_new));
+            TRY(v_axpby(c, ps, p, 1.0, ps, g, gam_new / gam, ps, &p, nullptr));   // p = g + (gam'/gam) p
+            gam = gam_new;
+        }
+        if (!converged) {   // fold what we have
+            TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
+        }
+    }
+    c->iterations = k;
+    // S10: x_e = A^{-1} (b_e - D_eo x_o)
+    TRY(op_schur_hop(c, PDd, 0, xhi, be, te));
+    TRY(op_Ainv(c, PDd, te, rhi));                                          // rhi now holds x_e
+    CUDA_OK(c, mdwf_launch_full_out(PDd, rhi, sol_dev, 8, c->L, c->L5, 0, c->st));
+    CUDA_OK(c, mdwf_launch_full_out(PDd, xhi, sol_dev, 8, c->L, c->L5, 1, c->st));
+    c->launches += 2;
+    // true residual with the unpreconditioned operator, fp64: || b - D x || / || b ||
+    TRY(op_D_parity(c, PDd, 0, xhi, rhi, te));
+    TRY(op_D_parity(c, PDd, 1, rhi, xhi, bp));
+    double re2 = 0, ro2 = 0;
+    TRY(v_axpby(c, PDd, te, 1.0, PDd, be, -1.0, PDd, &te, &re2));
+    TRY(v_axpby(c, PDd, bp, 1.0, PDd, bo, -1.0, PDd, &bp, &ro2));
+    const double tr = std::sqrt(re2 + ro2) / bnorm;
+    c->true_residual = tr;
+    if (iters_out) *iters_out = k;
+    if (true_res_out) *true_res_out = tr;
+    if (!(tr <= tol * 1.0000001) && !converged) { c->err = "CG did not converge within maxiter"; return MDWF_ENOCONV; }
+    return MDWF_OK;
+}
+
+int mdwf_solve(mdwf_ctx *c, const void *src_dev, void *sol_dev, double tol, int maxiter, int *iters_out,
+               double *true_res_out)
+{
+    TRY(check_ready(c));
+    if (!src_dev || !sol_dev || src_dev == sol_dev || !(tol > 0.0) || maxiter < 0) { c->err = "mdwf_solve: bad argument"; return MDWF_EARG; }
+    cudaEvent_t e0, e1;
+    CUDA_OK(c, cudaEventCreate(&e0));
+    CUDA_OK(c, cudaEventCreate(&e1));
+    CUDA_OK(c, cudaEventRecord(e0, c->st));
+    const int rc = solve_device(c, src_dev, sol_dev, tol, maxiter, iters_out, true_res_out);
+    cudaEventRecord(e1, c->st);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    c->solve_seconds = ms * 1e-3;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
+}
+
+int mdwf_solve_host(mdwf_ctx *c, const void *src_host, void *sol_host, double tol, int maxiter, int *iters_out,
+                    double *true_res_out)
+{
+    TRY(check_ready(c));
+    if (!src_host || !sol_host) return MDWF_EARG;
+    const size_t bytes = (size_t)2 * c->Vh * c->L5 * 24 * 8;
+    void *src = nullptr, *sol = nullptr;
+    TRY(get_raw(c, "host.src", bytes, &src));
+    TRY(get_raw(c, "host.sol", bytes, &sol));
+    CUDA_OK(c, cudaMemcpyAsync(src, src_host, bytes, cudaMemcpyHostToDevice, c->st));
+    const int rc = mdwf_solve(c, src, sol, tol, maxiter, iters_out, true_res_out);
+    if (rc != MDWF_OK && rc != MDWF_ENOCONV) return rc;
+    CUDA_OK(c, cudaMemcpyAsync(sol_host, sol, bytes, cudaMemcpyDeviceToHost, c->st));
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return rc;
+}
+
+// ---- S7 entry points on flat arrays ---------------------------------------------------------------------
+int mdwf_blas_norm2(mdwf_ctx *c, const void *x, long long n, int real_bytes, double *out)
+{
+    if (!c || !x || !out || n < 0 || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    TRY(ensure_scalars(c));
+    CUDA_OK(c, mdwf_launch_flat_reduce(0, x, x, n, real_bytes, c->partial, c->result_dev, c->st));
+    c->launches += 2;
+    return fetch_scalar(c, out);
+}
+int mdwf_blas_redot(mdwf_ctx *c, const void *x, const void *y, long long n, int real_bytes, double *out)
+{
+    if (!c || !x || !y || !out || n < 0 || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    TRY(ensure_scalars(c));
+    CUDA_OK(c, mdwf_launch_flat_reduce(1, x, y, n, real_bytes, c->partial, c->result_dev, c->st));
+    c->launches += 2;
+    return fetch_scalar(c, out);
+}
+int mdwf_blas_axpy(mdwf_ctx *c, double a, const void *x, void *y, long long n, int real_bytes)
+{
+    if (!c || !x || !y || n < 0 || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    CUDA_OK(c, mdwf_launch_flat_axpy(a, x, y, n, real_bytes, c->st));
+    c->launches += 1;
+    return MDWF_OK;
+}
+
+int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4)
+{
+    TRY(check_ready(c));
+    if (!precision || !out4 || reps < 1 || warmup < 0 || (op != MDWF_OP_MPC && op != MDWF_OP_MPCDAG)) return MDWF_EARG;
+    const std::string pr(precision);
+    Prec p;
+    if (pr == "fp64") p = PREC_D; else if (pr == "fp32") p = PREC_S; else if (pr == "half") p = PREC_H;
+    else { c->err = "precision must be fp64|fp32|half"; return MDWF_EARG; }
+    SpinorBuf a, t, b;
+    TRY(get_spinor(c, "tm.a", p, &a));
+    TRY(get_spinor(c, "tm.t", p, &t));
+    TRY(get_spinor(c, "tm.b", p, &b));
+    CUDA_OK(c, mdwf_launch_fill(p, a, c->L5, c->Vh, 12345u, c->st));
+    CUDA_OK(c, mdwf_launch_fill(p, t, c->L5, c->Vh, 999u, c->st));
+    c->launches += 2;
+    cudaEvent_t e0, e1;
+    CUDA_OK(c, cudaEventCreate(&e0));
+    CUDA_OK(c, cudaEventCreate(&e1));
+    const double l0 = c->launches;
+    for (int phase = 0; phase < 3; phase++) {     // 0: K1 + K2 back to back, 1: K1 alone, 2: K2 alone
+        for (int it = -warmup; it < reps; it++) {
+            if (it == 0) CUDA_OK(c, cudaEventRecord(e0, c->st));
+            if (phase != 2) TRY(op == MDWF_OP_MPC ? op_Mpc_k1(c, p, a, t) : op_Mpcdag_k1(c, p, a, t));
+            if (phase != 1) TRY(op == MDWF_OP_MPC ? op_Mpc_k2(c, p, a, t, b) : op_Mpcdag_k2(c, p, a, t, b));
+        }
+        CUDA_OK(c, cudaEventRecord(e1, c->st));
+        CUDA_OK(c, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CUDA_OK(c, cudaEventElapsedTime(&ms, e0, e1));
+        out4[phase] = (double)ms / reps;
+    }
+    out4[3] = c->launches - l0;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return MDWF_OK;
+}
+
+int mdwf_get_stat(const mdwf_ctx *c, const char *key, double *value)
+{
+    if (!c || !key || !value) return MDWF_EARG;
+    const std::string k(key);
+    if (k == "launches") *value = c->launches;
+    else if (k == "iterations") *value = c->iterations;
+    else if (k == "reliable_updates") *value = c->reliable_updates;
+    else if (k == "solve_seconds") *value = c->solve_seconds;
+    else if (k == "true_residual") *value = c->true_residual;
+    else if (k == "op_applications") *value = c->op_applications;
+    else if (k == "sloppy_applications") *value = c->sloppy_applications;
+    else return MDWF_EARG;
+    return MDWF_OK;
+}
+
+}   // extern "C"

@@ -1,0 +1,82 @@
+// mdwf_internal.h -- host-side declarations shared by the translation units of libmdwf_b200.so.
+// Device layouts:
+//   parity spinor, precision P:  chunk[(s*NV + j)*Vh + cb], chunk = double2 (fp64, NV=12, one complex),
+//                                float4 (fp32, NV=6, two complex) or short4 (16-bit fixed point, NV=6)
+//                                with one float scale norm[s*Vh + cb] per 5D site for the 16-bit format.
+//   gauge, per parity p of the site the link starts from: link[(mu*NK + k)*Vh + cb], one complex per
+//                                chunk (double2 / float2 / short2), NK = 9 (18 reals) or 6 (12 reals).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+enum Prec { PREC_D = 0, PREC_S = 1, PREC_H = 2 };
+
+struct SpinorBuf {       // one single-parity 5D vector in a device layout
+    void *v = nullptr;
+    float *norm = nullptr;   // 16-bit format only
+};
+
+struct HopArgs {
+    int L[4];
+    int L5;
+    int Vh;
+    int parity_out;          // parity of the sites this launch writes
+    const void *in;          // hop input: vector on the opposite parity
+    const float *in_norm;
+    const void *own;         // own-site input (same parity as the output) or nullptr
+    const float *own_norm;
+    void *out;
+    float *out_norm;
+    const void *gauge_same;  // links starting at sites of parity_out      (forward hops)
+    const void *gauge_other; // links starting at sites of the other parity (backward hops)
+    int recon;               // 18 or 12
+    double coef_hop;         // multiplies the hop sum
+    double pre_d, pre_o;     // PRE = 1: input is (pre_d + pre_o Lambda) psi        (B on load)
+    double own_d, own_o;     // OWN = 2/3: adds (own_d + own_o Lambda[^dagger]) psi_own
+    double post_d, post_o;   // POST = 2: applies (post_d + post_o Lambda^dagger) to coef_hop * hop
+    double mf;
+    const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
+};
+
+// hop family launcher.  dag: 0 H, 1 H^dagger.  pre: 0 none, 1 B on load.  post: 0 none, 1 dense
+// s-matrix, 2 bidiagonal Lambda^dagger form.  own: 0 none, 1 + psi_own, 2 + (d + o Lambda) psi_own,
+// 3 + (d + o Lambda^dagger) psi_own.  Returns cudaError_t as int.
+int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st);
+
+// site-local dense s-matrix: out = M in (M = R[2][L5][L5] on device, in the precision's compute type)
+int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, const void *dense,
+                       cudaStream_t st);
+
+// BLAS-1 on parity vectors: out = a x + b y (y may be null when b == 0); if partial != nullptr also the
+// deterministic reduction ||out||^2 -> *result_dev (double).  Mixed precisions allowed.
+int mdwf_launch_axpby(Prec po, const SpinorBuf &out, double a, Prec px, const SpinorBuf &x, double b, Prec py,
+                      const SpinorBuf &y, int L5, int Vh, double *partial, double *result_dev, cudaStream_t st);
+// reductions on parity vectors: kind 0: ||x||^2, 1: Re<x,y>
+int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const SpinorBuf &y, int L5, int Vh,
+                       double *partial, double *result_dev, cudaStream_t st);
+int mdwf_reduce_max_blocks();
+
+// flat-array BLAS-1 (mdwf_blas_* entry points)
+int mdwf_launch_flat_reduce(int kind, const void *x, const void *y, long long n, int real_bytes, double *partial,
+                            double *result_dev, cudaStream_t st);
+int mdwf_launch_flat_axpy(double a, const void *x, void *y, long long n, int real_bytes, cudaStream_t st);
+
+// layout conversion.  canonical parity spinor [s][cb][12 complex] <-> device layout
+int mdwf_launch_parity_in(Prec p, const void *canon, int real_bytes, const SpinorBuf &dst, int L5, int Vh,
+                          cudaStream_t st);
+int mdwf_launch_parity_out(Prec p, const SpinorBuf &src, void *canon, int real_bytes, int L5, int Vh,
+                           cudaStream_t st);
+// canonical full 5D spinor [s][t][z][y][x][12 complex] <-> one parity in the device layout
+int mdwf_launch_full_in(Prec p, const void *canon, int real_bytes, const SpinorBuf &dst, const int *L, int L5,
+                        int parity, cudaStream_t st);
+int mdwf_launch_full_out(Prec p, const SpinorBuf &src, void *canon, int real_bytes, const int *L, int L5,
+                         int parity, cudaStream_t st);
+// canonical gauge U[t][z][y][x][mu][3][3] -> device layout of one parity
+int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, const int *L, int parity, int recon,
+                         cudaStream_t st);
+
+// deterministic pseudo-random fill in [-1,1] (timing inputs only)
+int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st);
+
+size_t mdwf_spinor_bytes(Prec p, int L5, int Vh);   // bytes of the chunk array
+size_t mdwf_gauge_bytes(Prec p, int Vh, int recon); // bytes of one parity's link array
