@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py -- the measurement contract.
+
+A "step" is one pass of the whole hot path: one mdwf_solve (Schur preparation, mixed-precision CG on
+Mpc^+ Mpc with reliable updates to tol 1e-10, reconstruction, fp64 true residual) of the headline workload
+BASELINE.json quotes its metric on: configs[3] = 32^3 x 96, L5 = 12, double/single/half ladder, 12-real links,
+synthetic exp(i 0.1 H) links, Gaussian source.  `value` is the sustained operator TFLOP/s over the step
+(the paper's Table VI quantity) at the fixed count 2880 + 48 L5 flop per odd 5D site per
+Mpc / Mpc^+ application; the Dslash (Mpc) GB/s and TFLOP/s per precision and the solve seconds are in
+"mpc" and "solve".  Multi-GPU = replicas only: every rank solves its own right-hand side, no collective on
+the data path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload 0..4]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "mdwf_eo_dslash_sustained_tflops_in_mixed_precision_cg_solve"
+UNIT = "TFLOP/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for ln in self.f.read().splitlines():
+            c = [v.strip() for v in ln.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg, U_host, b_host, n_tslices, steps=1, warmup=0):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: Mpc then Mpc^+ (the operator work
+    of one CG iteration) evaluated on the odd sites of the first n_tslices time slices of the lattice."""
+    import numpy as np
+    from oracle import mdwf_oracle as mo
+    L, L5 = cfg["L"], cfg["L5"]
+    orc = mo.MdwfOracle(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], U_host)
+    Lx, Ly, Lz, Lt = L
+    sites = orc.sites_odd[orc.sites_odd < Lx * Ly * Lz * n_tslices]
+    v = orc.parity_part(b_host, 1) if b_host.shape == orc.shape else b_host
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        orc.Mpc(v, sites)
+        orc.Mpcdag(v, sites)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    flops = 2.0 * mo.flops_per_site(L5) * len(sites) * L5
+    sec = sum(times) / len(times)
+    return {"value": flops / sec / 1e12, "unit": UNIT, "cores": mo.num_threads(), "kind": "oracle",
+            "sample": "Mpc + Mpc^dagger (operator work of one CG iteration) on the odd sites of %d of %d time "
+                      "slices of %s (%d 5D sites), %.2f s per pass, halo sites recomputed"
+                      % (n_tslices, Lt, cfg["name"], len(sites) * L5, sec),
+            "seconds_per_pass": sec}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle timed on the host cores (rank 0 only), same config / metric / unit."""
+    if rank != 0:
+        return
+    import torch
+    from paper_1701_07559_b200 import inputs
+    cfg = inputs.CONFIGS[args.workload]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    U = inputs.gauge_field(cfg["L"], cfg["eps"], cfg["seed"], device=dev).cpu().numpy()
+    b = inputs.gaussian_source(cfg["L"], cfg["L5"], cfg["seed"], device=dev).cpu().numpy()
+    nts = min(cfg["L"][3], args.ref_tslices)
+    r = oracle_sample(cfg, U, b, nts, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_pass"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, args),
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args):
+    return {"workload": "BASELINE.json configs[%d]: %s, M5=%g b5=%g c5=%g m_f=%g, links exp(i %g H) seed %d, "
+                        "Gaussian source, ladder %s, reconstruct %d, tol 1e-10"
+                        % (args.workload, cfg["name"], cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], cfg["eps"],
+                           cfg["seed"], cfg["ladder"], cfg["reconstruct"]),
+            "parallelism": "replicas only: one right-hand side per GPU, no data-path collective",
+            "l2": "every vector of the step (>= 0.9 GB) is larger than the 126 MB L2; no explicit flush"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--workload", type=int, default=3, help="index into BASELINE.json configs (default 3 = 32^3x96xL5=12)")
+    ap.add_argument("--ref-tslices", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--op-reps", type=int, default=20)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1701_07559_b200 import binding, build, inputs
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = inputs.CONFIGS[args.workload]
+    L, L5 = cfg["L"], cfg["L5"]
+    Vh = L[0] * L[1] * L[2] * L[3] // 2
+    h = Vh * L5
+    hbm_peak, peak_src = measured_peaks()
+
+    # ---- inputs: same gauge field on every rank, one right-hand side per rank ---------------------------
+    U = inputs.gauge_field(L, cfg["eps"], cfg["seed"], device="cuda")
+    src = inputs.gaussian_source(L, L5, cfg["seed"] + 17 * rank, device="cuda")
+    m = binding.Mdwf(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"])
+    m.set_option("reconstruct", cfg["reconstruct"])
+    m.set_option("ladder", cfg["ladder"])
+    m.load_gauge(U)
+    F = m.flops_per_site()
+    sol = torch.empty_like(src)
+    tol, maxiter = 1e-10, 100000
+
+    def one_solve(host=False, s=None, x=None):
+        s = src if s is None else s
+        x = sol if x is None else x
+        rc, it, tr = binding.mdwf_solve(m.h, s.data_ptr(), x.data_ptr(), tol, maxiter, host=host)
+        if rc != 0 or not (tr <= tol * 1.001):
+            raise SystemExit("solve failed: rc=%d true residual %.3e" % (rc, tr))
+        return it, tr, m.stat("op_applications"), m.stat("solve_seconds")
+
+    # ---- device-resident steps -----------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        one_solve()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    l0 = m.stat("launches")
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    apps = 0
+    for _ in range(args.steps):
+        it, tr, na, _ = one_solve()
+        apps += na
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = m.stat("launches") - l0
+    ms_total = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    a = torch.tensor([apps], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+    ms_total, apps_all = float(t.item()), float(a.item())
+    value = apps_all * F * h / (ms_total * 1e-3) / 1e12
+    iters, true_res, n_upd = it, tr, m.stat("reliable_updates")
+
+    # ---- end to end: host buffers, H2D of the source and D2H of the solution inside the timed region ----------
+    src_h = src.cpu().pin_memory()
+    sol_h = torch.empty_like(src_h).pin_memory()
+    one_solve(True, src_h, sol_h)
+    barrier()
+    t0 = time.perf_counter()
+    apps_e = 0
+    for _ in range(args.steps):
+        apps_e += one_solve(True, src_h, sol_h)[2]
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    a = torch.tensor([apps_e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+    e2e_value = float(a.item()) * F * h / float(t.item()) / 1e12
+    nbytes = src_h.numel() * 16
+
+    # ---- per-kernel Dslash numbers and the roofline of the dominant kernel -------------------------------------
+    gl = {18: {"fp64": 8, "fp32": 4, "half": 2}, 12: {"fp64": 8, "fp32": 4, "half": 2}}
+    recon = int(cfg["reconstruct"])
+    mpc = {}
+    for prec, rb, extra in (("fp64", 8, 0), ("fp32", 4, 0), ("half", 2, 4)):
+        # two-pass algorithmic bytes per odd 5D site: K1 reads psi, writes t; K2 reads t, psi,
+        # writes out (5 spinor streams) + 2 hops x 8 links x recon reals / L5 (+ one fp32 scale per 16-bit spinor)
+        b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
+        for op, name in ((binding.OP_MPC, "Mpc"), (binding.OP_MPCDAG, "Mpcdag")):
+            r = m.time_op(op, prec, reps=args.op_reps, warmup=3)
+            mpc["%s_%s" % (name, prec)] = {
+                "ms": r["ms"], "ms_k1": r["ms_k1"], "ms_k2": r["ms_k2"],
+                "tflops": F * h / (r["ms"] * 1e-3) / 1e12,
+                "GBs_model": b_site * h / (r["ms"] * 1e-3) / 1e9,
+                "frac_hbm": b_site * h / (r["ms"] * 1e-3) / 1e9 / hbm_peak,
+                "bytes_per_site_model": b_site}
+    sloppy = {"d": "fp64", "ds": "fp32", "dh": "half", "dsh": "half"}[cfg["ladder"]]
+    rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[sloppy]
+    k1 = mpc["Mpc_%s" % sloppy]
+    k1_bytes = (2 * (24 * rb + extra) + 8 * recon * rb / L5) * h       # K1: read psi, write t, 8 links / L5
+    roofline = {"kernel": "hop_kernel<%s,PRE=B,POST=dense> (K1 of Mpc: t_e = B A^-1 H_eo B psi_o)" % sloppy,
+                "bound": "hbm", "achieved": k1_bytes / (k1["ms_k1"] * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "peak_source": peak_src, "traffic": None,
+                "algorithmic_bytes_per_launch": k1_bytes}
+    roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    tf = os.path.join(ROOT, "profiles", "traffic.json")      # dram bytes per launch from the committed ncu capture
+    if os.path.exists(tf):
+        try:
+            roofline["traffic"] = json.load(open(tf)).get("k1_%s_bytes_per_launch" % sloppy)
+        except Exception:
+            pass
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {"fp64": "f64", "fp32": "f32", "half": "i16 storage / f32 arithmetic"}[sloppy],
+            "data": "synthetic", "config": workload_config(cfg, args), "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                    "seconds_per_step": float(t.item()) / args.steps},
+            "gpu_launches": int(launches),
+            "solve": {"seconds": ms_total * 1e-3 / args.steps, "iterations": int(iters), "reliable_updates": int(n_upd),
+                      "true_residual": true_res, "op_applications_per_solve": apps / args.steps,
+                      "flops_per_site": F, "sites": h},
+            "mpc": mpc, "roofline": roofline}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nts = min(L[3], args.ref_tslices)
+        r = oracle_sample(cfg, U.cpu().numpy(), src_h.numpy(), nts)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    m.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

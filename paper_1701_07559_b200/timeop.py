@@ -1,0 +1,47 @@
+"""Time (or profile under ncu) the fused Mpc / Mpc^dagger kernels on one of BASELINE.json's workloads.
+
+  python -m paper_1701_07559_b200.timeop --workload 3 --prec fp32,half --reps 5 --warmup 2
+
+Prints one JSON line per (op, precision): ms per application and per kernel, model GB/s, TFLOP/s.
+Few launches, so it is the command the ncu captures under profiles/ are taken with.
+"""
+import argparse
+import json
+
+import torch
+
+from . import binding, build, inputs
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", type=int, default=3)
+    ap.add_argument("--prec", default="fp64,fp32,half")
+    ap.add_argument("--ops", default="0,1")
+    ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--reconstruct", default=None)
+    args = ap.parse_args()
+    build.build()
+    cfg = inputs.CONFIGS[args.workload]
+    L, L5 = cfg["L"], cfg["L5"]
+    recon = int(args.reconstruct or cfg["reconstruct"])
+    m = binding.Mdwf(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"])
+    m.set_option("reconstruct", recon)
+    m.load_gauge(inputs.gauge_field(L, cfg["eps"], cfg["seed"], device="cuda"))
+    torch.cuda.empty_cache()
+    h = L[0] * L[1] * L[2] * L[3] // 2 * L5
+    F = m.flops_per_site()
+    for prec in args.prec.split(","):
+        rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[prec]
+        b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
+        for op in (int(o) for o in args.ops.split(",")):
+            r = m.time_op(op, prec, reps=args.reps, warmup=args.warmup)
+            r.update(op=("Mpc", "Mpcdag")[op], prec=prec, workload=cfg["name"], reconstruct=recon,
+                     tflops=F * h / (r["ms"] * 1e-3) / 1e12, GBs_model=b_site * h / (r["ms"] * 1e-3) / 1e9)
+            print(json.dumps(r), flush=True)
+    m.close()
+
+
+if __name__ == "__main__":
+    main()
