@@ -71,18 +71,18 @@ axpby_kernel(void *out, float *out_norm, double a, const void *x, const float *x
         const int s = (int)(idx / Vh);
         const long cb = idx - (long)s * Vh;
         typename PX::R vx[24];
-        load_spinor<PX>(x, xn, s, cb, Vh, vx);
+        load_spinor<PX>(x, xn, L5, s, cb, vx);
         RO r[24];
         if (HASY) {
             typename PY::R vy[24];
-            load_spinor<PY>(y, yn, s, cb, Vh, vy);
+            load_spinor<PY>(y, yn, L5, s, cb, vy);
 #pragma unroll
             for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k] + b * (double)vy[k]);
         } else {
 #pragma unroll
             for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k]);
         }
-        store_spinor<PO>(out, out_norm, s, cb, Vh, r);
+        store_spinor<PO>(out, out_norm, L5, s, cb, r);
         if (NORM) {
 #pragma unroll
             for (int k = 0; k < 24; k++) sum += (double)r[k] * (double)r[k];
@@ -101,13 +101,13 @@ reduce_kernel(const void *x, const float *xn, const void *y, const float *yn, in
         const int s = (int)(idx / Vh);
         const long cb = idx - (long)s * Vh;
         typename PX::R vx[24];
-        load_spinor<PX>(x, xn, s, cb, Vh, vx);
+        load_spinor<PX>(x, xn, L5, s, cb, vx);
         if (KIND == 0) {
 #pragma unroll
             for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vx[k];
         } else {
             typename PY::R vy[24];
-            load_spinor<PY>(y, yn, s, cb, Vh, vy);
+            load_spinor<PY>(y, yn, L5, s, cb, vy);
 #pragma unroll
             for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vy[k];
         }

@@ -3,14 +3,15 @@
 #include "mdwf_device.cuh"
 #include "mdwf_internal.h"
 
+static size_t padded(int Vh) { return ((size_t)Vh + 31) / 32 * 32; }   // sites are stored in groups of 32
 size_t mdwf_spinor_bytes(Prec p, int L5, int Vh)
 {
-    const size_t n = (size_t)L5 * Vh * 24;
+    const size_t n = (size_t)L5 * padded(Vh) * 24;
     return p == PREC_D ? n * 8 : (p == PREC_S ? n * 4 : n * 2);
 }
 size_t mdwf_gauge_bytes(Prec p, int Vh, int recon)
 {
-    const size_t n = (size_t)4 * Vh * recon;
+    const size_t n = (size_t)4 * padded(Vh) * recon;
     return p == PREC_D ? n * 8 : (p == PREC_S ? n * 4 : n * 2);
 }
 
@@ -42,7 +43,7 @@ __global__ void spinor_in_kernel(const T *canon, void *dst, float *dst_norm, int
     R v[24];
 #pragma unroll
     for (int k = 0; k < 24; k++) v[k] = (R)p[k];
-    store_spinor<P>(dst, dst_norm, s, cb, Vh, v);
+    store_spinor<P>(dst, dst_norm, L5, s, cb, v);
 }
 template <class P, class T>
 __global__ void spinor_out_kernel(const void *src, const float *src_norm, T *canon, int L5, long Vh, int full,
@@ -56,7 +57,7 @@ __global__ void spinor_out_kernel(const void *src, const float *src_norm, T *can
     const long site = full ? ((long)s * V4 + cb_to_lex(cb, parity, Lx, Ly, Lz)) : idx;
     T *p = canon + site * 24;
     R v[24];
-    load_spinor<P>(src, src_norm, s, cb, Vh, v);
+    load_spinor<P>(src, src_norm, L5, s, cb, v);
 #pragma unroll
     for (int k = 0; k < 24; k++) p[k] = (T)v[k];
 }
@@ -79,8 +80,8 @@ __global__ void gauge_in_kernel(const T *canon, void *dst, long Vh, int parity, 
     const long lex = cb_to_lex(cb, parity, Lx, Ly, Lz);
     const T *p = canon + (lex * 4 + mu) * 18;
     const int NK = recon >> 1;
-    G *q = reinterpret_cast<G *>(dst) + ((long)mu * NK) * Vh + cb;
-    for (int k = 0; k < NK; k++) q[(long)k * Vh] = gpack((double)p[2 * k], (double)p[2 * k + 1], (G *)nullptr);
+    G *q = reinterpret_cast<G *>(dst) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
+    for (int k = 0; k < NK; k++) q[32 * k] = gpack((double)p[2 * k], (double)p[2 * k + 1], (G *)nullptr);
 }
 
 template <class P>
@@ -188,7 +189,7 @@ __global__ void fill_kernel(void *dst, float *dst_norm, int L5, long Vh, unsigne
         h ^= h >> 15; h *= 2246822519u; h ^= h >> 13; h *= 3266489917u; h ^= h >> 16;
         v[k] = (R)((double)h * (2.0 / 4294967295.0) - 1.0);
     }
-    store_spinor<P>(dst, dst_norm, s, cb, Vh, v);
+    store_spinor<P>(dst, dst_norm, L5, s, cb, v);
 }
 int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st)
 {

@@ -139,7 +139,7 @@ static int get_spinor(mdwf_ctx *c, const std::string &name, Prec p, SpinorBuf *o
     if (it != c->pool.end()) { *out = it->second; return MDWF_OK; }
     SpinorBuf b;
     CUDA_OK(c, cudaMalloc(&b.v, mdwf_spinor_bytes(p, c->L5, c->Vh)));
-    if (p == PREC_H) CUDA_OK(c, cudaMalloc((void **)&b.norm, sizeof(float) * (size_t)c->L5 * c->Vh));
+    if (p == PREC_H) CUDA_OK(c, cudaMalloc((void **)&b.norm, sizeof(float) * (size_t)c->L5 * ((c->Vh + 31) / 32 * 32)));
     c->pool[key] = b;
     *out = b;
     return MDWF_OK;
@@ -200,7 +200,7 @@ static int v_norm2(mdwf_ctx *c, Prec p, const SpinorBuf &x, double *out)
 static int v_zero(mdwf_ctx *c, Prec p, const SpinorBuf &x)
 {
     CUDA_OK(c, cudaMemsetAsync(x.v, 0, mdwf_spinor_bytes(p, c->L5, c->Vh), c->st));
-    if (p == PREC_H) CUDA_OK(c, cudaMemsetAsync(x.norm, 0, sizeof(float) * (size_t)c->L5 * c->Vh, c->st));
+    if (p == PREC_H) CUDA_OK(c, cudaMemsetAsync(x.norm, 0, sizeof(float) * (size_t)c->L5 * ((c->Vh + 31) / 32 * 32), c->st));
     return MDWF_OK;
 }
 
@@ -236,7 +236,7 @@ static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, con
 static int op_Mpc_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp)
 {
     HopArgs k1 = base_args(c, p, 0, in, nullptr, tmp);        // K1: t_e = (B A^{-1}) H_eo (B in_o)
-    k1.coef_hop = 1.0; k1.pre_d = c->b5; k1.pre_o = c->c5; k1.dense = dense_ptr(c, p, DENSE_BAINV);
+    k1.coef_hop = c->b5; k1.pre_d = c->b5; k1.pre_o = c->c5; k1.dense = dense_ptr(c, p, DENSE_BAINV);   // b5 of B-on-load folded in
     return run_hop(c, p, 0, 1, 1, 0, k1);
 }
 static int op_Mpc_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
@@ -279,7 +279,7 @@ static int op_D_parity(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_othe
                        const SpinorBuf &out)
 {
     HopArgs a = base_args(c, p, parity, in_other, &in_same, out);
-    a.coef_hop = -0.5; a.pre_d = c->b5; a.pre_o = c->c5; a.own_d = c->alpha; a.own_o = c->beta;
+    a.coef_hop = -0.5 * c->b5; a.pre_d = c->b5; a.pre_o = c->c5; a.own_d = c->alpha; a.own_o = c->beta;
     return run_hop(c, p, 0, 1, 0, 2, a);
 }
 // one parity of D^+: out_p = A^+ in_p - (1/2) B^+ H'_{p,pbar} in_pbar
@@ -295,7 +295,7 @@ static int op_schur_hop(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_oth
                         const SpinorBuf &out)
 {
     HopArgs a = base_args(c, p, parity, in_other, &own, out);
-    a.coef_hop = 0.5; a.pre_d = c->b5; a.pre_o = c->c5;
+    a.coef_hop = 0.5 * c->b5; a.pre_d = c->b5; a.pre_o = c->c5;
     return run_hop(c, p, 0, 1, 0, 1, a);
 }
 static int op_Ainv(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out)
@@ -332,7 +332,7 @@ int mdwf_create(mdwf_ctx **out, int Lx, int Ly, int Lz, int Lt, int L5, double M
     c->M5 = M5; c->b5 = b5; c->c5 = c5; c->mf = m_f;
     c->alpha = b5 * (4.0 - M5) + 1.0;
     c->beta = c5 * (4.0 - M5) - 1.0;
-    if (c->alpha == 0.0) { delete c; return MDWF_EARG; }
+    if (c->alpha == 0.0 || b5 == 0.0) { delete c; return MDWF_EARG; }   // A must be invertible; b5 is divided out on load
     *out = c;
     return MDWF_OK;
 }

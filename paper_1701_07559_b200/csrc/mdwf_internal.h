@@ -1,10 +1,11 @@
 // mdwf_internal.h -- host-side declarations shared by the translation units of libmdwf_b200.so.
 // Device layouts:
-//   parity spinor, precision P:  chunk[(s*NV + j)*Vh + cb], chunk = double2 (fp64, NV=12, one complex),
-//                                float4 (fp32, NV=6, two complex) or short4 (16-bit fixed point, NV=6)
-//                                with one float scale norm[s*Vh + cb] per 5D site for the 16-bit format.
-//   gauge, per parity p of the site the link starts from: link[(mu*NK + k)*Vh + cb], one complex per
-//                                chunk (double2 / float2 / short2), NK = 9 (18 reals) or 6 (12 reals).
+//   sites of one parity are grouped in 32s: g = cb >> 5, lane = cb & 31 (arrays padded to whole groups).
+//   parity spinor, precision P:  chunk[((g*L5 + s)*NV + j)*32 + lane], chunk = double2 (fp64, NV=12, one
+//                                complex), float4 (fp32, NV=6, two complex) or short4 (16-bit fixed point,
+//                                NV=6) with one float scale norm[(g*L5 + s)*32 + lane] per 5D site.
+//   gauge, per parity p of the site the link starts from: link[((g*4 + mu)*NK + k)*32 + lane], one complex
+//                                per chunk (double2 / float2 / short2), NK = 9 (18 reals) or 6 (12 reals).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
