@@ -100,7 +100,17 @@ __global__ void __launch_bounds__(HopCfg<P, S>::MAXT, HopCfg<P, S>::MINB) hop_ke
     const int L5 = L5T ? L5T : a.L5;
     const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
     const int NSG = L5 / S;
-    const long cb = (long)blockIdx.x * 32 + lane;
+    // Sweep order: the grid walks z-chunk by z-chunk and, inside a chunk, t-slice by
+    // t-slice, so that the t+-1 neighbours are re-read from L2 after one small slab, not after a whole t-slice.
+    long cb0 = (long)blockIdx.x * 32;
+    if (a.sweep_nb) {
+        const int Lt = a.L[3];
+        const int per_chunk = a.sweep_nb * Lt;
+        const int c = blockIdx.x / per_chunk, r = blockIdx.x - c * per_chunk;
+        const int t = r / a.sweep_nb, q = r - t * a.sweep_nb;
+        cb0 = (long)t * ((long)a.Vh / Lt) + (long)c * a.sweep_chunk + (long)q * 32;
+    }
+    const long cb = cb0 + lane;
     const bool active = cb < a.Vh;
     R *dense = tile + (size_t)L5 * 24 * 32;              // [2][L5][L5]       (POST == 1)
     if (POST == 1) {

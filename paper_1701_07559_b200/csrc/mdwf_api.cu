@@ -50,6 +50,7 @@ struct mdwf_ctx {
     int apply_prec = -1;     // -1 auto
     double delta = 0.1;
     int max_update_interval = 0;
+    int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
     void *dense[2][DENSE_KINDS] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [0] double, [1] float
@@ -216,6 +217,18 @@ static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const Spinor
     a.L5 = c->L5;
     a.Vh = c->Vh;
     a.parity_out = parity_out;
+    // z-chunked sweep: ZC = largest divisor of Lz whose slab (3 spinor streams of ZC planes) stays under the budget
+    {
+        const long plane = (long)(c->L[0] / 2) * c->L[1];
+        const long rb = (p == PREC_D) ? 8 : (p == PREC_S ? 4 : 2);
+        const long budget = c->sweep_mb > 0 ? (long)c->sweep_mb << 20 : (16L << 20);
+        int zc = 0;
+        for (int d = 1; d <= c->L[2]; d++)
+            if (c->L[2] % d == 0 && (d * plane) % 32 == 0 && d * plane * 3 * c->L5 * 24 * rb <= budget) zc = d;
+        if (c->sweep_mb < 0 || zc == c->L[2] || zc < 2) zc = 0;
+        a.sweep_nb = zc ? (int)(zc * plane / 32) : 0;
+        a.sweep_chunk = (int)(zc * plane);
+    }
     a.in = in.v; a.in_norm = in.norm;
     a.own = own ? own->v : nullptr; a.own_norm = own ? own->norm : nullptr;
     a.out = out.v; a.out_norm = out.norm;
@@ -383,6 +396,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
         c->delta = d;
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
+    } else if (k == "sweep_mb") {
+        c->sweep_mb = atoi(value);
     } else if (k == "stream") {
         c->st = (cudaStream_t)(uintptr_t)strtoull(value, nullptr, 10);
     } else if (k == "matpc") {

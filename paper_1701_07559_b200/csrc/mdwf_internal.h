@@ -22,6 +22,8 @@ struct HopArgs {
     int L5;
     int Vh;
     int parity_out;          // parity of the sites this launch writes
+    int sweep_nb;            // block sweep order: blocks per (z-chunk, t) slab; 0 = plain lexicographic order
+    int sweep_chunk;         // sites per (z-chunk, t) slab = ZC * Ly * Lx/2
     const void *in;          // hop input: vector on the opposite parity
     const float *in_norm;
     const void *own;         // own-site input (same parity as the output) or nullptr

@@ -21,6 +21,7 @@ def main():
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--reconstruct", default=None)
+    ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value")
     args = ap.parse_args()
     build.build()
     cfg = inputs.CONFIGS[args.workload]
@@ -28,6 +29,8 @@ def main():
     recon = int(args.reconstruct or cfg["reconstruct"])
     m = binding.Mdwf(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"])
     m.set_option("reconstruct", recon)
+    for kv in args.opt:
+        m.set_option(*kv.split("=", 1))
     m.load_gauge(inputs.gauge_field(L, cfg["eps"], cfg["seed"], device="cuda"))
     torch.cuda.empty_cache()
     h = L[0] * L[1] * L[2] * L[3] // 2 * L5
