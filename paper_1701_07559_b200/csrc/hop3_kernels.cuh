@@ -1,0 +1,552 @@
+// hop3_kernels.cuh -- v3 of the fused Wilson-hopping + fifth-dimension kernels for fp32 ARITHMETIC
+// (precisions PS = fp32 storage and PH = 16-bit storage), L5 in {8, 12, 16}.
+//
+// Same operator family and same thread mapping as hop_kernels.cuh (thread = one 4D site x S consecutive
+// s-slices; block = 32 sites x L5/S warps), rebuilt around three B200 facts measured in profiles/:
+//   1. sm_100a issues a 3-register FFMA at half rate; the packed FFMA2 (fma.rn.f32x2) carries two FMAs per
+//      lane and reaches 65 TFLOP/s against 40 for FFMA.  A complex number is one float2 register pair and
+//      every arithmetic step below is a packed f32x2 instruction: SU(3) x half-spinor is
+//      chi_a = sum_c (ur,ur)*(hr,hi) + (-ui,ui)*(hi,hr); the links are expanded once per direction into those
+//      two pair forms and reused for the S slices and both spin components.
+//   2. The dense L5 x L5 matrix B A^{-1} (S3 of the hot path) is semiseparable: A = alpha (1 + kappa T) with T
+//      the cyclic shift carrying -m_f at the wall, so A^{-1} is a first-order recurrence plus a rank-one wall
+//      term.  Each thread runs the recurrence over its own S slices in registers, the warps of a block
+//      exchange ONE carry per component through shared memory, and
+//          t_s = (b5 z_s + c5 z_{s-1}) / alpha + qW_s W,    z_s = x_s - kappa z_{s-1},  W = z_{L5-1}
+//      replaces 2 L5 FMAs per real by about 6 (DESIGN.md section 5 derives it; the fp64 path and any L5 outside
+//      {8,12,16} keep the dense table of hop_kernels.cuh).
+//   3. No register spills: the s-window of the B-on-load stencil slides slice by slice.
+#pragma once
+#include "mdwf_device.cuh"
+#include "mdwf_internal.h"
+
+namespace h3 {
+
+typedef float2 c2;   // one complex number = one packed f32x2 operand
+MDWF_DEV c2 fma2(c2 a, c2 b, c2 c) { return __ffma2_rn(a, b, c); }
+MDWF_DEV c2 add2(c2 a, c2 b) { return __fadd2_rn(a, b); }
+MDWF_DEV c2 mul2(c2 a, c2 b) { return __fmul2_rn(a, b); }
+MDWF_DEV c2 dup(float a) { return make_float2(a, a); }
+MDWF_DEV c2 swp(c2 a) { return make_float2(a.y, a.x); }
+MDWF_DEV c2 mk(float a, float b) { return make_float2(a, b); }
+
+// ---- spinor chunk loads into complex pairs ------------------------------------------------------
+// PS: chunk j = float4 = complexes 2j, 2j+1.  PH: chunk j = short4, value = scale * int16.
+template <class P> struct Ld;
+template <> struct Ld<PS> {
+    // NC complexes (NC even) from chunk pointer p (stride 32 chunks)
+    template <int NC> static MDWF_DEV void chunks(const float4 *p, float, c2 *v)
+    {
+#pragma unroll
+        for (int j = 0; j < NC / 2; j++) {
+            const float4 q = __ldg(p + 32 * j);
+            v[2 * j] = mk(q.x, q.y);
+            v[2 * j + 1] = mk(q.z, q.w);
+        }
+    }
+};
+template <> struct Ld<PH> {
+    template <int NC> static MDWF_DEV void chunks(const short4 *p, float sc, c2 *v)
+    {
+        const c2 s2 = dup(sc);
+#pragma unroll
+        for (int j = 0; j < NC / 2; j++) {
+            const short4 q = __ldg(p + 32 * j);
+            v[2 * j] = mul2(s2, mk((float)q.x, (float)q.y));
+            v[2 * j + 1] = mul2(s2, mk((float)q.z, (float)q.w));
+        }
+    }
+};
+
+// ---- links in pair form -----------------------------------------------------------------------------
+// M = U (forward hop) or U^dagger (backward hop), entry (a,c):  R[a*3+c] = (re, re),  I[a*3+c] = (-im, im).
+struct Link {
+    c2 R[9], I[9];
+};
+MDWF_DEV void gget(const float2 q, float &re, float &im) { re = q.x; im = q.y; }
+MDWF_DEV void gget(const short2 q, float &re, float &im)
+{
+    re = (float)q.x * (1.0f / MDWF_FIXED_MAX);
+    im = (float)q.y * (1.0f / MDWF_FIXED_MAX);
+}
+// stage one link (as stored: 6 or 9 complex chunks) from global into the block's shared-memory link table
+template <class P>
+MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, typename P::G *dst)
+{
+    using G = typename P::G;
+    const int NK = recon >> 1;
+    const G *p = reinterpret_cast<const G *>(gbase) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
+    G tmp[9];
+#pragma unroll
+    for (int k = 0; k < 6; k++) tmp[k] = __ldg(p + 32 * k);
+    if (recon == 18) {
+#pragma unroll
+        for (int k = 6; k < 9; k++) tmp[k] = __ldg(p + 32 * k);
+    }
+#pragma unroll
+    for (int k = 0; k < 6; k++) dst[32 * k] = tmp[k];
+    if (recon == 18) {
+#pragma unroll
+        for (int k = 6; k < 9; k++) dst[32 * k] = tmp[k];
+    }
+}
+// p = this lane's column of the shared-memory link table of one direction (element k at p[32 k])
+template <class P, bool DAGGER>
+MDWF_DEV void load_link3(const typename P::G *p, int recon, Link &L)
+{
+    float ur[9], ui[9];
+#pragma unroll
+    for (int k = 0; k < 6; k++) gget(p[32 * k], ur[k], ui[k]);
+    if (recon == 18) {
+#pragma unroll
+        for (int k = 6; k < 9; k++) gget(p[32 * k], ur[k], ui[k]);
+    } else {
+        // row2[c] = conj(row0[a] row1[b] - row0[b] row1[a]),  (a,b) = (c+1, c+2) mod 3
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const int a = (c + 1) % 3, b = (c + 2) % 3;
+            float re = ur[a] * ur[3 + b];
+            re = fmaf(-ui[a], ui[3 + b], re); re = fmaf(-ur[b], ur[3 + a], re); re = fmaf(ui[b], ui[3 + a], re);
+            float im = ur[a] * ui[3 + b];
+            im = fmaf(ui[a], ur[3 + b], im); im = fmaf(-ur[b], ui[3 + a], im); im = fmaf(-ui[b], ur[3 + a], im);
+            ur[6 + c] = re;
+            ui[6 + c] = -im;
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            if (!DAGGER) {
+                L.R[a * 3 + c] = dup(ur[a * 3 + c]);
+                L.I[a * 3 + c] = mk(-ui[a * 3 + c], ui[a * 3 + c]);
+            } else {   // (U^dagger)_{ac} = conj(U_{ca})
+                L.R[a * 3 + c] = dup(ur[c * 3 + a]);
+                L.I[a * 3 + c] = mk(ui[c * 3 + a], -ui[c * 3 + a]);
+            }
+        }
+}
+
+// chi[sp*3+a] = sum_c M[a][c] h[sp*3+c]: 6 FMUL2-started chains of 6 packed ops
+MDWF_DEV void su3_mul3(const Link &L, const c2 *h, c2 *chi)
+{
+    c2 hs[6];
+#pragma unroll
+    for (int k = 0; k < 6; k++) hs[k] = swp(h[k]);
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            c2 acc = mul2(L.R[a * 3], h[sp * 3]);
+            acc = fma2(L.I[a * 3], hs[sp * 3], acc);
+#pragma unroll
+            for (int c = 1; c < 3; c++) {
+                acc = fma2(L.R[a * 3 + c], h[sp * 3 + c], acc);
+                acc = fma2(L.I[a * 3 + c], hs[sp * 3 + c], acc);
+            }
+            chi[sp * 3 + a] = acc;
+        }
+}
+
+// ---- spin projection / reconstruction in the DeGrand-Rossi basis, complex-pair form ----------------
+// v[spin*3+colour].  (1 - SGN gamma_mu) v has upper half h (returned) and a lower half that follows from h:
+//   mu=0: h0 = v0 - S i v3, h1 = v1 - S i v2;  r2 =  S i h1, r3 =  S i h0
+//   mu=1: h0 = v0 + S v3,   h1 = v1 - S v2;    r2 = -S h1,   r3 =  S h0
+//   mu=2: h0 = v0 - S i v2, h1 = v1 + S i v3;  r2 =  S i h0, r3 = -S i h1
+//   mu=3: h0 = v0 - S v2,   h1 = v1 - S v3;    r2 = -S h0,   r3 = -S h1
+// -S i (a + i b) = S (b, -a) = swp(.) * (S, -S);   S i (a + i b) = swp(.) * (-S, S).
+template <int MU, int SGN>
+MDWF_DEV void project3(const c2 *v, c2 *h)
+{
+    const float S = (float)SGN;
+    const c2 pm = mk(S, -S), mp = mk(-S, S), ss = mk(S, S), mm = mk(-S, -S);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if (MU == 0) {
+            h[c] = fma2(swp(v[9 + c]), pm, v[c]);
+            h[3 + c] = fma2(swp(v[6 + c]), pm, v[3 + c]);
+        } else if (MU == 1) {
+            h[c] = fma2(v[9 + c], ss, v[c]);
+            h[3 + c] = fma2(v[6 + c], mm, v[3 + c]);
+        } else if (MU == 2) {
+            h[c] = fma2(swp(v[6 + c]), pm, v[c]);
+            h[3 + c] = fma2(swp(v[9 + c]), mp, v[3 + c]);
+        } else {
+            h[c] = fma2(v[6 + c], mm, v[c]);
+            h[3 + c] = fma2(v[9 + c], mm, v[3 + c]);
+        }
+    }
+}
+// acc += sc * [chi ; lower(chi)],  sc = +-1 (antiperiodic t hop), acc[spin*3+colour]
+template <int MU, int SGN, bool WITHSC>
+MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
+{
+    const float p = WITHSC ? sc : 1.0f, S = (float)SGN * p;
+    const c2 pp = mk(p, p), mp = mk(-S, S), pm = mk(S, -S), ss = mk(S, S), mm = mk(-S, -S);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if (WITHSC) {
+            acc[c] = fma2(chi[c], pp, acc[c]);
+            acc[3 + c] = fma2(chi[3 + c], pp, acc[3 + c]);
+        } else {
+            acc[c] = add2(acc[c], chi[c]);
+            acc[3 + c] = add2(acc[3 + c], chi[3 + c]);
+        }
+        if (MU == 0) {
+            acc[6 + c] = fma2(swp(chi[3 + c]), mp, acc[6 + c]);
+            acc[9 + c] = fma2(swp(chi[c]), mp, acc[9 + c]);
+        } else if (MU == 1) {
+            acc[6 + c] = fma2(chi[3 + c], mm, acc[6 + c]);
+            acc[9 + c] = fma2(chi[c], ss, acc[9 + c]);
+        } else if (MU == 2) {
+            acc[6 + c] = fma2(swp(chi[c]), mp, acc[6 + c]);
+            acc[9 + c] = fma2(swp(chi[3 + c]), pm, acc[9 + c]);
+        } else {
+            acc[6 + c] = fma2(chi[c], mm, acc[6 + c]);
+            acc[9 + c] = fma2(chi[3 + c], mm, acc[9 + c]);
+        }
+    }
+}
+
+// ---- one direction of the stencil for the S slices of this thread ----------------------------------
+// FWD: neighbour x+mu through U_mu(x); else neighbour x-mu through U_mu(x-mu)^dagger.
+// PRE = 1 applies (1 + f Lambda) to the neighbour on load: upper spins add f * (slice s-1), lower spins
+// f * (slice s+1), wall factor -m_f at the wrap.  The window slides over the S slices (one half-spinor of
+// halo on each side), so only one full slice and two half slices are live at a time.
+template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR>
+MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const typename P::G *sl, long cb_nb, float bsign,
+                        c2 (*acc)[12], long cb_pf = -1)
+{
+    using V = typename P::V;
+    constexpr int SGN = (FWD ? 1 : -1) * (DAG ? -1 : 1);
+    Link U;
+    load_link3<P, !FWD>(sl, a.recon, U);
+
+    const V *p0 = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, s0);
+    const long n0 = sp_noff(L5, cb_nb, s0);
+    constexpr long SL = 32 * P::NV;
+
+    if (PRE == 0) {
+#pragma unroll
+        for (int k = 0; k < S; k++) {
+            c2 v[12], h[6], chi[6];
+            Ld<P>::template chunks<12>(p0 + k * SL, load_scale<P>(a.in_norm, n0 + 32 * k), v);
+            project3<MU, SGN>(v, h);
+            su3_mul3(U, h, chi);
+            recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
+        }
+    } else {
+        const float f = (float)(a.pre_o / a.pre_d), fw = (float)(-a.mf * a.pre_o / a.pre_d);
+        const int sm = (s0 == 0) ? L5 - 1 : s0 - 1;
+        const int sp = (s0 + S >= L5) ? 0 : s0 + S;
+        c2 prev_up[6], cur[12], nxt[12];
+        {
+            const V *pm = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, sm);
+            Ld<P>::template chunks<6>(pm, load_scale<P>(a.in_norm, sp_noff(L5, cb_nb, sm)), prev_up);
+        }
+        Ld<P>::template chunks<12>(p0, load_scale<P>(a.in_norm, n0), cur);
+#pragma unroll
+        for (int k = 0; k < S; k++) {
+            if (k < S - 1) {
+                Ld<P>::template chunks<12>(p0 + (k + 1) * SL, load_scale<P>(a.in_norm, n0 + 32 * (k + 1)), nxt);
+            } else {
+                const V *pp = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, sp) + 32 * (P::NV / 2);
+                Ld<P>::template chunks<6>(pp, load_scale<P>(a.in_norm, sp_noff(L5, cb_nb, sp)), nxt + 6);
+            }
+            const c2 fu = dup((s0 + k == 0) ? fw : f);
+            const c2 fl = dup((s0 + k == L5 - 1) ? fw : f);
+            c2 w[12], h[6], chi[6];
+#pragma unroll
+            for (int q = 0; q < 6; q++) {
+                w[q] = fma2(fu, prev_up[q], cur[q]);
+                w[6 + q] = fma2(fl, nxt[6 + q], cur[6 + q]);
+            }
+            project3<MU, SGN>(w, h);
+            su3_mul3(U, h, chi);
+            recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
+#pragma unroll
+            for (int q = 0; q < 6; q++) prev_up[q] = cur[q];
+            if (k < S - 1) {
+#pragma unroll
+                for (int q = 0; q < 12; q++) cur[q] = nxt[q];
+            }
+        }
+    }
+}
+
+// ---- spinor store from complex pairs ---------------------------------------------------------------
+template <class P> MDWF_DEV void store3(void *base, float *norm, int L5, int s, long cb, const c2 *o);
+template <> MDWF_DEV void store3<PS>(void *base, float *, int L5, int s, long cb, const c2 *o)
+{
+    float4 *p = reinterpret_cast<float4 *>(base) + sp_off(L5, PS::NV, cb, s);
+#pragma unroll
+    for (int j = 0; j < 6; j++) p[32 * j] = make_float4(o[2 * j].x, o[2 * j].y, o[2 * j + 1].x, o[2 * j + 1].y);
+}
+template <> MDWF_DEV void store3<PH>(void *base, float *norm, int L5, int s, long cb, const c2 *o)
+{
+    short4 *p = reinterpret_cast<short4 *>(base) + sp_off(L5, PH::NV, cb, s);
+    float m = 0.f;
+#pragma unroll
+    for (int q = 0; q < 12; q++) m = fmaxf(m, fmaxf(fabsf(o[q].x), fabsf(o[q].y)));
+    norm[sp_noff(L5, cb, s)] = m;
+    const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f);
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const c2 e = mul2(o[2 * j], isc), f = mul2(o[2 * j + 1], isc);
+        p[32 * j] = make_short4((short)__float2int_rn(e.x), (short)__float2int_rn(e.y), (short)__float2int_rn(f.x),
+                                (short)__float2int_rn(f.y));
+    }
+}
+
+// ---- fifth-dimension epilogues on the S slices of a thread -----------------------------------------
+// Orientation: "direct" (MIRROR = false) is the P+ pattern of A = alpha + beta Lambda (slice s couples to s-1);
+// MIRROR = true is the P- pattern (s couples to s+1), i.e. the same recurrence with s -> L5-1-s.
+// Effective index of a thread's slice k:  j = MIRROR ? S-1-k : k,  of its warp: g = MIRROR ? NSG-1-sg : sg.
+
+// local recurrence z_j = x_j - kappa z_{j-1} (z_{-1} = 0) in place on components [off, off+6)
+template <int S, bool MIRROR>
+MDWF_DEV void rec_local(c2 (*x)[12], int off, c2 nk)
+{
+#pragma unroll
+    for (int j = 1; j < S; j++) {
+        const int k = MIRROR ? S - 1 - j : j, kp = MIRROR ? k + 1 : k - 1;
+#pragma unroll
+        for (int q = 0; q < 6; q++) x[k][off + q] = fma2(nk, x[kp][off + q], x[k][off + q]);
+    }
+}
+// t_j = bz z_j + cz z_{j-1} + qC_j C + qW_s W  in place (j descending so that z_{j-1} is still the local value)
+template <int S, int NSG, bool MIRROR>
+MDWF_DEV void rec_finish(c2 (*x)[12], int off, int sg, const c2 *sE, int lane, const HopArgs &a)
+{
+    const int g = MIRROR ? NSG - 1 - sg : sg;
+    const c2 cS = dup(a.r_cpow);
+    c2 C[6], W[6];
+#pragma unroll
+    for (int q = 0; q < 6; q++) { C[q] = mk(0.f, 0.f); W[q] = mk(0.f, 0.f); }
+#pragma unroll
+    for (int j = 0; j < NSG; j++) {          // Horner over the carries of the warps in effective order
+        const int jj = MIRROR ? NSG - 1 - j : j;
+        if (j == g) {
+#pragma unroll
+            for (int q = 0; q < 6; q++) C[q] = W[q];
+        }
+#pragma unroll
+        for (int q = 0; q < 6; q++) W[q] = fma2(cS, W[q], sE[(jj * 12 + off + q) * 32 + lane]);
+    }
+    const c2 bz = dup(a.r_bz), cz = dup(a.r_cz);
+#pragma unroll
+    for (int j = S - 1; j >= 0; j--) {
+        const int k = MIRROR ? S - 1 - j : j, kp = MIRROR ? k + 1 : k - 1;
+        const c2 qC = dup(a.r_qC[j]), qW = dup(a.r_qW[g * S + j]);
+#pragma unroll
+        for (int q = 0; q < 6; q++) {
+            c2 t = mul2(bz, x[k][off + q]);
+            if (j > 0) t = fma2(cz, x[kp][off + q], t);
+            t = fma2(qC, C[q], t);
+            x[k][off + q] = fma2(qW, W[q], t);
+        }
+    }
+}
+
+template <class P, int S> struct Hop3Cfg {
+    // 8 warps per SM (two blocks of 128 threads or one of 256): up to 255 registers per thread
+    static constexpr int WARPS = MDWF_H3_WARPS;    // resident warps per SM asked of ptxas
+};
+
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+__global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S) > 0 ? Hop3Cfg<P, S>::WARPS / (L5 / S) : 1) hop3_kernel(const HopArgs a)
+{
+    constexpr int NSG = L5 / S;
+    using V = typename P::V;
+    extern __shared__ __align__(16) unsigned char smem_raw3[];
+    c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
+    typename P::G *sL = reinterpret_cast<typename P::G *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
+    const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
+    long cb0 = (long)blockIdx.x * 32;
+    if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
+        const int Lt = a.L[3];
+        const int per_chunk = a.sweep_nb * Lt;
+        const int c = blockIdx.x / per_chunk, r = blockIdx.x - c * per_chunk;
+        const int t = r / a.sweep_nb, q = r - t * a.sweep_nb;
+        cb0 = (long)t * ((long)a.Vh / Lt) + (long)c * a.sweep_chunk + (long)q * 32;
+    }
+    const long cb = cb0 + lane;
+    const bool active = cb < a.Vh;
+
+    c2 acc[S][12];
+#pragma unroll
+    for (int k = 0; k < S; k++)
+#pragma unroll
+        for (int q = 0; q < 12; q++) acc[k][q] = mk(0.f, 0.f);
+
+    // neighbour indices (inactive lanes of a ragged last block keep cb = 0 and load nothing)
+    const long cbs = active ? cb : 0;
+    const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
+    int r = (int)cbs;
+    const int xh = r % Lxh; r /= Lxh;
+    const int y = r % Ly;   r /= Ly;
+    const int z = r % Lz;
+    const int t = r / Lz;
+    const int xodd = (a.parity_out + y + z + t) & 1;
+    const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
+    long nb[8];
+    nb[0] = xodd ? (xh == Lxh - 1 ? cbs - (Lxh - 1) : cbs + 1) : cbs;
+    nb[1] = xodd ? cbs : (xh == 0 ? cbs + (Lxh - 1) : cbs - 1);
+    nb[2] = (y == Ly - 1) ? cbs - (Ly - 1) * sy : cbs + sy;
+    nb[3] = (y == 0) ? cbs + (Ly - 1) * sy : cbs - sy;
+    nb[4] = (z == Lz - 1) ? cbs - (Lz - 1) * sz : cbs + sz;
+    nb[5] = (z == 0) ? cbs + (Lz - 1) * sz : cbs - sz;
+    nb[6] = (t == Lt - 1) ? cbs - (Lt - 1) * st : cbs + st;
+    nb[7] = (t == 0) ? cbs + (Lt - 1) * st : cbs - st;
+    const float btp = (t == Lt - 1) ? -1.f : 1.f;               // antiperiodic in t
+    const float btm = (t == 0) ? -1.f : 1.f;
+
+    // stage the 8 links of the block's 32 sites in shared memory once: direction d = 2 mu + (0 fwd, 1 bwd) is
+    // fetched by warp d mod NSG; the NSG warps of a site then read them from there (no per-direction global
+    // latency on the critical path, 1/NSG of the global link loads)
+    if (active) {
+#pragma unroll
+        for (int d = 0; d < 8; d++)
+            if ((d % NSG) == sg) {
+                if ((d & 1) == 0) stage_link<P>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
+                else stage_link<P>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
+            }
+    }
+    __syncthreads();
+
+    if (active) {
+        hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, nb[0], 1.f, acc);
+        hop_dir3<P, 0, false, DAG, PRE, S, false>(a, L5, s0, sL + 1 * 288 + lane, nb[1], 1.f, acc);
+        hop_dir3<P, 1, true, DAG, PRE, S, false>(a, L5, s0, sL + 2 * 288 + lane, nb[2], 1.f, acc);
+        hop_dir3<P, 1, false, DAG, PRE, S, false>(a, L5, s0, sL + 3 * 288 + lane, nb[3], 1.f, acc);
+        hop_dir3<P, 2, true, DAG, PRE, S, false>(a, L5, s0, sL + 4 * 288 + lane, nb[4], 1.f, acc);
+        hop_dir3<P, 2, false, DAG, PRE, S, false>(a, L5, s0, sL + 5 * 288 + lane, nb[5], 1.f, acc);
+        hop_dir3<P, 3, true, DAG, PRE, S, true>(a, L5, s0, sL + 6 * 288 + lane, nb[6], btp, acc);
+        hop_dir3<P, 3, false, DAG, PRE, S, true>(a, L5, s0, sL + 7 * 288 + lane, nb[7], btm, acc);
+    }
+
+    if (POST == 1) {
+        // coef_hop * (B A^{-1}) acc per chirality (DAG: the transposed pattern) by blocked recurrence
+        const c2 nk = dup(a.r_nk);
+        rec_local<S, DAG != 0>(acc, 0, nk);              // upper spins: direct pattern (mirrored for the dagger)
+        rec_local<S, DAG == 0>(acc, 6, nk);              // lower spins: mirrored pattern (direct for the dagger)
+        constexpr int kU = DAG ? 0 : S - 1, kL = DAG ? S - 1 : 0;    // slice holding the carry-out
+#pragma unroll
+        for (int q = 0; q < 6; q++) {
+            sE[(sg * 12 + q) * 32 + lane] = acc[kU][q];
+            sE[(sg * 12 + 6 + q) * 32 + lane] = acc[kL][6 + q];
+        }
+        __syncthreads();
+        rec_finish<S, NSG, DAG != 0>(acc, 0, sg, sE, lane, a);
+        rec_finish<S, NSG, DAG == 0>(acc, 6, sg, sE, lane, a);
+    } else if (POST == 2) {
+        // coef_hop * (post_d + post_o Lambda^dagger) acc: upper spins take s+1, lower spins s-1, -m_f at the wrap
+#pragma unroll
+        for (int q = 0; q < 6; q++) {
+            sE[(sg * 12 + q) * 32 + lane] = acc[0][q];               // first slice, upper: halo of warp sg-1
+            sE[(sg * 12 + 6 + q) * 32 + lane] = acc[S - 1][6 + q];   // last slice, lower: halo of warp sg+1
+        }
+        __syncthreads();
+        const int gu = (sg == NSG - 1) ? 0 : sg + 1, gl = (sg == 0) ? NSG - 1 : sg - 1;
+        const float coef = (float)a.coef_hop, o = coef * (float)a.post_o, ow = -o * (float)a.mf;
+        const c2 d2 = dup(coef * (float)a.post_d), o2 = dup(o);
+        const c2 ou = dup(sg == NSG - 1 ? ow : o), ol = dup(sg == 0 ? ow : o);
+#pragma unroll
+        for (int k = 0; k < S; k++)
+#pragma unroll
+            for (int q = 0; q < 6; q++) {
+                const c2 nb = (k < S - 1) ? acc[k + 1][q] : sE[(gu * 12 + q) * 32 + lane];
+                acc[k][q] = fma2(d2, acc[k][q], mul2((k < S - 1) ? o2 : ou, nb));
+            }
+#pragma unroll
+        for (int k = S - 1; k >= 0; k--)
+#pragma unroll
+            for (int q = 0; q < 6; q++) {
+                const c2 nb = (k > 0) ? acc[k - 1][6 + q] : sE[(gl * 12 + 6 + q) * 32 + lane];
+                acc[k][6 + q] = fma2(d2, acc[k][6 + q], mul2((k > 0) ? o2 : ol, nb));
+            }
+    }
+    if (!active) return;
+
+    const c2 coef2 = dup(POST == 0 ? (float)a.coef_hop : 1.0f);     // POST != 0: coef_hop is already folded in
+#pragma unroll
+    for (int k = 0; k < S; k++) {
+        const int s = s0 + k;
+        c2 o[12];
+        if (OWN == 0) {
+#pragma unroll
+            for (int q = 0; q < 12; q++) o[q] = (POST == 0) ? mul2(coef2, acc[k][q]) : acc[k][q];
+        } else if (OWN == 1) {
+            c2 w[12];
+            const V *p = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, s);
+            Ld<P>::template chunks<12>(p, load_scale<P>(a.own_norm, sp_noff(L5, cb, s)), w);
+#pragma unroll
+            for (int q = 0; q < 12; q++) o[q] = fma2(coef2, acc[k][q], w[q]);
+        } else {
+            // (own_d + own_o Lambda) psi: upper from s-1, lower from s+1; Lambda^dagger (OWN == 3): swapped
+            c2 w[12], u[6], l[6];
+            const V *p = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, s);
+            Ld<P>::template chunks<12>(p, load_scale<P>(a.own_norm, sp_noff(L5, cb, s)), w);
+            int su = (OWN == 2) ? s - 1 : s + 1;
+            int sl = (OWN == 2) ? s + 1 : s - 1;
+            float fu = (float)a.own_o, fl = (float)a.own_o;
+            if (su < 0) { su = L5 - 1; fu *= (float)(-a.mf); }
+            if (su >= L5) { su = 0; fu *= (float)(-a.mf); }
+            if (sl < 0) { sl = L5 - 1; fl *= (float)(-a.mf); }
+            if (sl >= L5) { sl = 0; fl *= (float)(-a.mf); }
+            const V *pu = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, su);
+            const V *pl = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, sl) + 32 * (P::NV / 2);
+            Ld<P>::template chunks<6>(pu, load_scale<P>(a.own_norm, sp_noff(L5, cb, su)), u);
+            Ld<P>::template chunks<6>(pl, load_scale<P>(a.own_norm, sp_noff(L5, cb, sl)), l);
+            const c2 d2 = dup((float)a.own_d), fu2 = dup(fu), fl2 = dup(fl);
+#pragma unroll
+            for (int q = 0; q < 6; q++) {
+                o[q] = fma2(coef2, acc[k][q], fma2(d2, w[q], mul2(fu2, u[q])));
+                o[6 + q] = fma2(coef2, acc[k][6 + q], fma2(d2, w[6 + q], mul2(fl2, l[q])));
+            }
+        }
+        store3<P>(a.out, a.out_norm, L5, s, cb, o);
+    }
+}
+
+// ---- launchers ----------------------------------------------------------------------------------
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
+{
+    constexpr int NSG = L5 / S;
+    dim3 block(32, NSG);
+    dim3 grid((unsigned)((a.Vh + 31) / 32));
+    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(typename P::G);
+    hop3_kernel<P, DAG, PRE, POST, OWN, L5, S><<<grid, block, smem, st>>>(a);
+    return (int)cudaGetLastError();
+}
+template <class P, int DAG, int PRE, int POST, int OWN>
+static int launch_hop3_l5(const HopArgs &a, cudaStream_t st)
+{
+    if (a.L5 == 12) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 12, MDWF_H3_S12>(a, st);
+#ifndef MDWF_DEV_FAST
+    if (a.L5 == 8) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 8, 2>(a, st);
+    if (a.L5 == 16) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 16, 2>(a, st);
+#endif
+    return (int)cudaErrorInvalidValue;
+}
+// true when the v3 family covers this launch (fp32 arithmetic, tabulated L5, |kappa| < 1 for the recurrence)
+static inline bool hop3_supports(int L5, int post, const HopArgs &a)
+{
+    if (!(L5 == 8 || L5 == 12 || L5 == 16)) return false;
+    if (post == 1 && !(a.r_ok)) return false;
+    return true;
+}
+template <class P>
+static int launch_hop3_prec(int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
+{
+    if (!dag && pre == 1 && post == 1 && own == 0) return launch_hop3_l5<P, 0, 1, 1, 0>(a, st);   // K1
+    if (!dag && pre == 0 && post == 0 && own == 2) return launch_hop3_l5<P, 0, 0, 0, 2>(a, st);   // K2
+    if (!dag && pre == 1 && post == 0 && own == 2) return launch_hop3_l5<P, 0, 1, 0, 2>(a, st);   // D
+    if (!dag && pre == 1 && post == 0 && own == 1) return launch_hop3_l5<P, 0, 1, 0, 1>(a, st);   // Schur prep/recon
+    if (dag && pre == 0 && post == 1 && own == 0) return launch_hop3_l5<P, 1, 0, 1, 0>(a, st);    // K1^+
+    if (dag && pre == 0 && post == 2 && own == 3) return launch_hop3_l5<P, 1, 0, 2, 3>(a, st);    // K2^+, D^+
+    return (int)cudaErrorInvalidValue;
+}
+
+}   // namespace h3

@@ -15,12 +15,19 @@
 int mdwf_launch_hop_D(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_S(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 
 int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
 {
+    if (a.kver >= 3 && p != PREC_D) {        // v3 family (fp32 arithmetic); -1 = not covered, fall back to v2
+        const int rc = (p == PREC_S) ? mdwf_launch_hop3_S(dag, pre, post, own, a, st)
+                                     : mdwf_launch_hop3_H(dag, pre, post, own, a, st);
+        if (rc != -1) return rc;
+    }
     switch (p) {
     case PREC_D: return mdwf_launch_hop_D(dag, pre, post, own, a, st);
     case PREC_S: return mdwf_launch_hop_S(dag, pre, post, own, a, st);
@@ -50,6 +57,7 @@ struct mdwf_ctx {
     int apply_prec = -1;     // -1 auto
     double delta = 0.1;
     int max_update_interval = 0;
+    int kver = 3;            // kernel family for fp32 arithmetic: 3 = hop3_kernels.cuh, 2 = hop_kernels.cuh
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
@@ -238,8 +246,26 @@ static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const Spinor
     a.mf = c->mf;
     return a;
 }
-static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, const HopArgs &a)
+// constants of the recurrence form of coef_hop * B A^{-1} (hop3_kernels.cuh)
+static void fill_recurrence(const mdwf_ctx *c, HopArgs &a)
 {
+    const double ka = c->beta / c->alpha, nk = -ka, coef = a.coef_hop;
+    const int S = mdwf_h3_slices(c->L5);
+    a.r_ok = (std::fabs(ka) < 0.98) ? 1 : 0;
+    a.r_nk = (float)nk;
+    a.r_cpow = (float)std::pow(nk, S);
+    a.r_bz = (float)(coef * c->b5 / c->alpha);
+    a.r_cz = (float)(coef * c->c5 / c->alpha);
+    for (int j = 0; j < 4; j++)
+        a.r_qC[j] = (float)(coef * (c->b5 * std::pow(nk, j + 1) + c->c5 * std::pow(nk, j)) / c->alpha);
+    const double g = 1.0 / (c->alpha * (1.0 + c->mf * std::pow(nk, c->L5)));
+    for (int s = 0; s < 32; s++)
+        a.r_qW[s] = (s < c->L5) ? (float)(coef * (-g * c->mf) * (c->b5 * std::pow(nk, s + 1) + c->c5 * std::pow(nk, s))) : 0.f;
+}
+static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, HopArgs a)
+{
+    a.kver = c->kver;
+    if (post == 1 && p != PREC_D && a.kver >= 3) fill_recurrence(c, a);
     CUDA_OK(c, mdwf_launch_hop(p, dag, pre, post, own, a, c->st));
     c->launches += 1;
     return MDWF_OK;
@@ -396,6 +422,9 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
         c->delta = d;
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
+    } else if (k == "kernels") {
+        if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
+        else { c->err = "kernels must be v2|v3"; return MDWF_EARG; }
     } else if (k == "sweep_mb") {
         c->sweep_mb = atoi(value);
     } else if (k == "stream") {

@@ -10,6 +10,15 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// slices per thread of the v3 kernels (hop3_kernels.cuh) for L5 = 12, and resident warps per SM asked of ptxas
+#ifndef MDWF_H3_S12
+#define MDWF_H3_S12 3
+#endif
+#ifndef MDWF_H3_WARPS
+#define MDWF_H3_WARPS 8
+#endif
+static inline int mdwf_h3_slices(int L5) { return L5 == 12 ? MDWF_H3_S12 : 2; }
+
 enum Prec { PREC_D = 0, PREC_S = 1, PREC_H = 2 };
 
 struct SpinorBuf {       // one single-parity 5D vector in a device layout
@@ -39,6 +48,14 @@ struct HopArgs {
     double post_d, post_o;   // POST = 2: applies (post_d + post_o Lambda^dagger) to coef_hop * hop
     double mf;
     const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
+    // POST = 1 in the v3 kernels (hop3_kernels.cuh): coef_hop * B A^{-1} as a blocked recurrence
+    int kver;                // host side: kernel family requested (2 or 3)
+    int r_ok;                // 1 when the recurrence form is usable (|kappa| < 1)
+    float r_nk;              // -kappa = -beta/alpha
+    float r_cpow;            // (-kappa)^S, S = slices per thread
+    float r_bz, r_cz;        // coef_hop b5/alpha, coef_hop c5/alpha
+    float r_qC[4];           // coef_hop (b5 p_j + c5 p_{j-1})/alpha, p_j = (-kappa)^{j+1}, p_{-1} = 1
+    float r_qW[32];          // coef_hop * wall term of slice s (effective index): -g m_f (b5 (-kappa)^{s+1} + c5 (-kappa)^s)
 };
 
 // hop family launcher.  dag: 0 H, 1 H^dagger.  pre: 0 none, 1 B on load.  post: 0 none, 1 dense
