@@ -45,15 +45,24 @@ template <> struct Ld<PS> {
         }
     }
 };
+// 16-bit fixed point -> fp32 without the conversion pipe: 0x4B400000 | (q ^ 0x8000) is the float 12582912 + 32768 + q,
+// so value = (that - 12615680) * scale, both steps exact up to the one rounding of the product: one LOP3 per
+// word, one PRMT per value, one FADD2 + one FMUL2 per complex.
+MDWF_DEV c2 cvt_pair(unsigned w, c2 sc)      // w = two int16 (low half = first)
+{
+    const unsigned x = w ^ 0x80008000u;
+    const c2 f = mk(__uint_as_float(__byte_perm(x, 0x4B400000u, 0x7610)), __uint_as_float(__byte_perm(x, 0x4B400000u, 0x7632)));
+    return mul2(add2(f, dup(-12615680.0f)), sc);
+}
 template <> struct Ld<PH> {
     template <int NC> static MDWF_DEV void chunks(const short4 *p, float sc, c2 *v)
     {
         const c2 s2 = dup(sc);
 #pragma unroll
         for (int j = 0; j < NC / 2; j++) {
-            const short4 q = __ldg(p + 32 * j);
-            v[2 * j] = mul2(s2, mk((float)q.x, (float)q.y));
-            v[2 * j + 1] = mul2(s2, mk((float)q.z, (float)q.w));
+            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p + 32 * j));
+            v[2 * j] = cvt_pair(q.x, s2);
+            v[2 * j + 1] = cvt_pair(q.y, s2);
         }
     }
 };
@@ -66,8 +75,10 @@ struct Link {
 MDWF_DEV void gget(const float2 q, float &re, float &im) { re = q.x; im = q.y; }
 MDWF_DEV void gget(const short2 q, float &re, float &im)
 {
-    re = (float)q.x * (1.0f / MDWF_FIXED_MAX);
-    im = (float)q.y * (1.0f / MDWF_FIXED_MAX);
+    const unsigned w = ((unsigned)(unsigned short)q.y << 16) | (unsigned short)q.x;
+    const c2 v = cvt_pair(w, dup(1.0f / MDWF_FIXED_MAX));
+    re = v.x;
+    im = v.y;
 }
 // stage one link (as stored: 6 or 9 complex chunks) from global into the block's shared-memory link table
 template <class P>
@@ -289,12 +300,14 @@ template <> MDWF_DEV void store3<PH>(void *base, float *norm, int L5, int s, lon
 #pragma unroll
     for (int q = 0; q < 12; q++) m = fmaxf(m, fmaxf(fabsf(o[q].x), fabsf(o[q].y)));
     norm[sp_noff(L5, cb, s)] = m;
-    const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f);
+    // fp32 -> 16-bit fixed point by the magic-number add: the low 16 bits of fma(v, isc, 1.5 * 2^23) are round(v isc)
+    const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f), magic = dup(12582912.0f);
+    uint2 *pw = reinterpret_cast<uint2 *>(p);
 #pragma unroll
     for (int j = 0; j < 6; j++) {
-        const c2 e = mul2(o[2 * j], isc), f = mul2(o[2 * j + 1], isc);
-        p[32 * j] = make_short4((short)__float2int_rn(e.x), (short)__float2int_rn(e.y), (short)__float2int_rn(f.x),
-                                (short)__float2int_rn(f.y));
+        const c2 e = fma2(o[2 * j], isc, magic), f = fma2(o[2 * j + 1], isc, magic);
+        pw[32 * j] = make_uint2(__byte_perm(__float_as_uint(e.x), __float_as_uint(e.y), 0x5410),
+                                __byte_perm(__float_as_uint(f.x), __float_as_uint(f.y), 0x5410));
     }
 }
 
@@ -350,7 +363,9 @@ MDWF_DEV void rec_finish(c2 (*x)[12], int off, int sg, const c2 *sE, int lane, c
 
 template <class P, int S> struct Hop3Cfg {
     // 8 warps per SM (two blocks of 128 threads or one of 256): up to 255 registers per thread
-    static constexpr int WARPS = MDWF_H3_WARPS;    // resident warps per SM asked of ptxas
+    // resident warps per SM asked of ptxas: 8 (255 registers) for fp32 storage, whose 16-byte loads in flight need
+    // the registers; 12 (168 registers) for 16-bit storage
+    static constexpr int WARPS = P::HALF ? MDWF_H3_WARPS_H : MDWF_H3_WARPS;
 };
 
 template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>

@@ -17,6 +17,9 @@
 #ifndef MDWF_H3_WARPS
 #define MDWF_H3_WARPS 8
 #endif
+#ifndef MDWF_H3_WARPS_H
+#define MDWF_H3_WARPS_H 12
+#endif
 static inline int mdwf_h3_slices(int L5) { return L5 == 12 ? MDWF_H3_S12 : 2; }
 
 enum Prec { PREC_D = 0, PREC_S = 1, PREC_H = 2 };
