@@ -15,7 +15,7 @@ OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG = 0, 1, 2, 3, 4
 
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
-           "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op"]
+           "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates"]
 
 _lib = None
 
@@ -51,6 +51,7 @@ def lib():
         L.mdwf_last_error.restype = ctypes.c_char_p
         L.mdwf_flops_per_site.argtypes = [P]
         L.mdwf_time_op.argtypes = [P, I, ctypes.c_char_p, I, I, ctypes.POINTER(D)]
+        L.mdwf_fma_rates.argtypes = [P, ctypes.POINTER(D)]
         _lib = L
     return _lib
 
@@ -169,6 +170,12 @@ class Mdwf:
 
     def time_op(self, op, precision, reps=20, warmup=3):
         return mdwf_time_op(self.h, op, precision, reps, warmup)
+
+    def fma_rates(self):
+        """(FFMA, FFMA2) rates of this device in 1e12 FMA/s (mdwf_fma_rates)."""
+        out = (ctypes.c_double * 2)()
+        _check(self.h, lib().mdwf_fma_rates(self.h, out))
+        return out[0], out[1]
 
     def norm2(self, x):
         v = ctypes.c_double(0.0)

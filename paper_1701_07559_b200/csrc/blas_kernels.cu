@@ -50,6 +50,12 @@ __global__ void final_sum_kernel(const double *partial, int n, double *result)
     }
 }
 
+int mdwf_launch_final_sum(const double *partial, int n, double *result_dev, cudaStream_t st)
+{
+    final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, n, result_dev);
+    return (int)cudaGetLastError();
+}
+
 static int red_blocks(long long work)
 {
     long long b = (work + RED_THREADS - 1) / RED_THREADS;
@@ -192,6 +198,53 @@ int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const Spi
     case PREC_D: return reduce_y<PD>(kind, py, x, y, L5, Vh, partial, result_dev, st);
     case PREC_S: return reduce_y<PS>(kind, py, x, y, L5, Vh, partial, result_dev, st);
     default: return reduce_y<PH>(kind, py, x, y, L5, Vh, partial, result_dev, st);
+    }
+}
+
+// ---- fused CG update: x += a p ; p = g + b p  (one read of p instead of two) --------------------------
+template <class PX, class PP>
+__global__ void __launch_bounds__(RED_THREADS)
+xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, const void *g, const float *gn, int L5, long Vh)
+{
+    const long n5 = (long)L5 * Vh;
+    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
+        const int s = (int)(idx / Vh);
+        const long cb = idx - (long)s * Vh;
+        typename PP::R vp[24], vg[24];
+        typename PX::R vx[24];
+        load_spinor<PP>(p, pn, L5, s, cb, vp);
+        load_spinor<PP>(g, gn, L5, s, cb, vg);
+        load_spinor<PX>(x, xn, L5, s, cb, vx);
+#pragma unroll
+        for (int k = 0; k < 24; k++) {
+            vx[k] = (typename PX::R)((double)vx[k] + a * (double)vp[k]);
+            vp[k] = (typename PP::R)((double)vg[k] + b * (double)vp[k]);
+        }
+        store_spinor<PX>(x, xn, L5, s, cb, vx);
+        store_spinor<PP>(p, pn, L5, s, cb, vp);
+    }
+}
+template <class PX>
+static int xpupdate_p(Prec pp, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g, int L5, int Vh,
+                      cudaStream_t st)
+{
+    const int nb = red_blocks((long long)L5 * Vh);
+#define XP(PP) xpupdate_kernel<PX, PP><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, L5, Vh)
+    switch (pp) {
+    case PREC_D: XP(PD); break;
+    case PREC_S: XP(PS); break;
+    default: XP(PH); break;
+    }
+#undef XP
+    return (int)cudaGetLastError();
+}
+int mdwf_launch_xpupdate(Prec px, const SpinorBuf &x, double a, Prec pp, const SpinorBuf &p, double b, const SpinorBuf &g,
+                         int L5, int Vh, cudaStream_t st)
+{
+    switch (px) {
+    case PREC_D: return xpupdate_p<PD>(pp, x, a, p, b, g, L5, Vh, st);
+    case PREC_S: return xpupdate_p<PS>(pp, x, a, p, b, g, L5, Vh, st);
+    default: return xpupdate_p<PH>(pp, x, a, p, b, g, L5, Vh, st);
     }
 }
 

@@ -286,14 +286,19 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const typename P::G *sl
 }
 
 // ---- spinor store from complex pairs ---------------------------------------------------------------
-template <class P> MDWF_DEV void store3(void *base, float *norm, int L5, int s, long cb, const c2 *o);
-template <> MDWF_DEV void store3<PS>(void *base, float *, int L5, int s, long cb, const c2 *o)
+// returns the sum of squares of the values as stored (for the fused norm of the output vector)
+template <class P> MDWF_DEV float store3(void *base, float *norm, int L5, int s, long cb, const c2 *o);
+template <> MDWF_DEV float store3<PS>(void *base, float *, int L5, int s, long cb, const c2 *o)
 {
     float4 *p = reinterpret_cast<float4 *>(base) + sp_off(L5, PS::NV, cb, s);
 #pragma unroll
     for (int j = 0; j < 6; j++) p[32 * j] = make_float4(o[2 * j].x, o[2 * j].y, o[2 * j + 1].x, o[2 * j + 1].y);
+    c2 n2 = mul2(o[0], o[0]);
+#pragma unroll
+    for (int q = 1; q < 12; q++) n2 = fma2(o[q], o[q], n2);
+    return n2.x + n2.y;
 }
-template <> MDWF_DEV void store3<PH>(void *base, float *norm, int L5, int s, long cb, const c2 *o)
+template <> MDWF_DEV float store3<PH>(void *base, float *norm, int L5, int s, long cb, const c2 *o)
 {
     short4 *p = reinterpret_cast<short4 *>(base) + sp_off(L5, PH::NV, cb, s);
     float m = 0.f;
@@ -303,12 +308,19 @@ template <> MDWF_DEV void store3<PH>(void *base, float *norm, int L5, int s, lon
     // fp32 -> 16-bit fixed point by the magic-number add: the low 16 bits of fma(v, isc, 1.5 * 2^23) are round(v isc)
     const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f), magic = dup(12582912.0f);
     uint2 *pw = reinterpret_cast<uint2 *>(p);
+    const c2 nmagic = dup(-12582912.0f);
+    c2 n2 = mk(0.f, 0.f);
 #pragma unroll
     for (int j = 0; j < 6; j++) {
         const c2 e = fma2(o[2 * j], isc, magic), f = fma2(o[2 * j + 1], isc, magic);
         pw[32 * j] = make_uint2(__byte_perm(__float_as_uint(e.x), __float_as_uint(e.y), 0x5410),
                                 __byte_perm(__float_as_uint(f.x), __float_as_uint(f.y), 0x5410));
+        const c2 qe = add2(e, nmagic), qf = add2(f, nmagic);      // the stored integers, exactly
+        n2 = fma2(qe, qe, n2);
+        n2 = fma2(qf, qf, n2);
     }
+    const float sc = m * (1.0f / MDWF_FIXED_MAX);
+    return (n2.x + n2.y) * sc * sc;
 }
 
 // ---- fifth-dimension epilogues on the S slices of a thread -----------------------------------------
@@ -481,8 +493,8 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
                 acc[k][6 + q] = fma2(d2, acc[k][6 + q], mul2((k > 0) ? o2 : ol, nb));
             }
     }
-    if (!active) return;
-
+    float nsum = 0.f;
+    if (active) {
     const c2 coef2 = dup(POST == 0 ? (float)a.coef_hop : 1.0f);     // POST != 0: coef_hop is already folded in
 #pragma unroll
     for (int k = 0; k < S; k++) {
@@ -520,7 +532,24 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
                 o[6 + q] = fma2(coef2, acc[k][6 + q], fma2(d2, w[6 + q], mul2(fl2, l[q])));
             }
         }
-        store3<P>(a.out, a.out_norm, L5, s, cb, o);
+        nsum += store3<P>(a.out, a.out_norm, L5, s, cb, o);
+    }
+    }
+    if (a.partial) {
+        // fused ||out||^2 (S7): fp32 per thread, then a fixed shuffle tree and a fixed order over the warps in fp64;
+        // one partial per block, summed in fixed order by final_sum_kernel -> bit-reproducible
+        __shared__ double wsum[NSG];
+        double v = (double)nsum;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) wsum[sg] = v;
+        __syncthreads();
+        if (lane == 0 && sg == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int j = 0; j < NSG; j++) t += wsum[j];
+            a.partial[blockIdx.x] = t;
+        }
     }
 }
 

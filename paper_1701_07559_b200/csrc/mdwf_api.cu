@@ -65,6 +65,7 @@ struct mdwf_ctx {
     std::map<std::string, SpinorBuf> pool;
     std::map<std::string, void *> raw;
     double *partial = nullptr, *result_dev = nullptr, *result_host = nullptr;
+    double *hop_partial = nullptr;   // one ||out||^2 partial per block of a hop launch (fused norms)
     // stats
     double launches = 0, iterations = 0, reliable_updates = 0, solve_seconds = 0, true_residual = 0;
     double op_applications = 0, sloppy_applications = 0;
@@ -176,6 +177,7 @@ static int ensure_scalars(mdwf_ctx *c)
     if (c->partial) return MDWF_OK;
     CUDA_OK(c, cudaMalloc((void **)&c->partial, sizeof(double) * mdwf_reduce_max_blocks()));
     CUDA_OK(c, cudaMalloc((void **)&c->result_dev, sizeof(double) * 4));
+    CUDA_OK(c, cudaMalloc((void **)&c->hop_partial, sizeof(double) * (size_t)((c->Vh + 31) / 32)));
     CUDA_OK(c, cudaMallocHost((void **)&c->result_host, sizeof(double) * 4));
     return MDWF_OK;
 }
@@ -278,16 +280,34 @@ static int op_Mpc_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &
     k1.coef_hop = c->b5; k1.pre_d = c->b5; k1.pre_o = c->c5; k1.dense = dense_ptr(c, p, DENSE_BAINV);   // b5 of B-on-load folded in
     return run_hop(c, p, 0, 1, 1, 0, k1);
 }
-static int op_Mpc_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+// the v3 kernels can emit ||out||^2 partials from their epilogue (fused norm)
+static bool fused_norm_available(const mdwf_ctx *c, Prec p)
+{
+    return p != PREC_D && c->kver >= 3 && (c->L5 == 8 || c->L5 == 12 || c->L5 == 16);
+}
+static int finish_norm(mdwf_ctx *c, Prec p, const SpinorBuf &out, bool fused, double *norm2_out)
+{
+    if (!norm2_out) return MDWF_OK;
+    if (!fused) return v_norm2(c, p, out, norm2_out);
+    CUDA_OK(c, mdwf_launch_final_sum(c->hop_partial, (c->Vh + 31) / 32, c->result_dev, c->st));
+    c->launches += 1;
+    return fetch_scalar(c, norm2_out);
+}
+static int op_Mpc_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out,
+                     double *norm2_out = nullptr)
 {
     HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2: out_o = A in_o - (1/4) H_oe t_e
     k2.coef_hop = -0.25; k2.own_d = c->alpha; k2.own_o = c->beta;
-    return run_hop(c, p, 0, 0, 0, 2, k2);
+    const bool fused = norm2_out && fused_norm_available(c, p);
+    if (fused) { TRY(ensure_scalars(c)); k2.partial = c->hop_partial; }
+    TRY(run_hop(c, p, 0, 0, 0, 2, k2));
+    return finish_norm(c, p, out, fused, norm2_out);
 }
-static int op_Mpc(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+static int op_Mpc(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out,
+                  double *norm2_out = nullptr)
 {
     TRY(op_Mpc_k1(c, p, in, tmp));
-    TRY(op_Mpc_k2(c, p, in, tmp, out));
+    TRY(op_Mpc_k2(c, p, in, tmp, out, norm2_out));
     c->op_applications += 1;
     if (p != PREC_D) c->sloppy_applications += 1;
     return MDWF_OK;
@@ -299,16 +319,21 @@ static int op_Mpcdag_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBu
     k1.coef_hop = 1.0; k1.dense = dense_ptr(c, p, DENSE_BAINV_DAG);
     return run_hop(c, p, 1, 0, 1, 0, k1);
 }
-static int op_Mpcdag_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+static int op_Mpcdag_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out,
+                        double *norm2_out = nullptr)
 {
     HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2+: out_o = A^+ in_o - (1/4) B^+ H'_oe u_e
     k2.coef_hop = -0.25; k2.post_d = c->b5; k2.post_o = c->c5; k2.own_d = c->alpha; k2.own_o = c->beta;
-    return run_hop(c, p, 1, 0, 2, 3, k2);
+    const bool fused = norm2_out && fused_norm_available(c, p);
+    if (fused) { TRY(ensure_scalars(c)); k2.partial = c->hop_partial; }
+    TRY(run_hop(c, p, 1, 0, 2, 3, k2));
+    return finish_norm(c, p, out, fused, norm2_out);
 }
-static int op_Mpcdag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+static int op_Mpcdag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out,
+                     double *norm2_out = nullptr)
 {
     TRY(op_Mpcdag_k1(c, p, in, tmp));
-    TRY(op_Mpcdag_k2(c, p, in, tmp, out));
+    TRY(op_Mpcdag_k2(c, p, in, tmp, out, norm2_out));
     c->op_applications += 1;
     if (p != PREC_D) c->sloppy_applications += 1;
     return MDWF_OK;
@@ -388,6 +413,7 @@ int mdwf_destroy(mdwf_ctx *c)
             if (c->dense[p][k]) cudaFree(c->dense[p][k]);
     if (c->partial) cudaFree(c->partial);
     if (c->result_dev) cudaFree(c->result_dev);
+    if (c->hop_partial) cudaFree(c->hop_partial);
     if (c->result_host) cudaFreeHost(c->result_host);
     delete c;
     return MDWF_OK;
@@ -588,18 +614,18 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
         TRY(v_axpby(c, ps, p, 1.0, ps, g, 0.0, ps, nullptr, &gam));         // p = g, gam = ||g||^2
         while (k < maxiter && !converged) {
             double qq = 0;
-            TRY(op_Mpc(c, ps, p, ts, q));                                   // q = Mpc p
-            TRY(v_norm2(c, ps, q, &qq));
+            TRY(op_Mpc(c, ps, p, ts, q, &qq));                              // q = Mpc p, ||q||^2 from the K2 epilogue
             if (!(qq > 0.0) || !(gam > 0.0)) break;
             const double a = gam / qq;
-            TRY(v_axpby(c, pxl, xlo, a, ps, p, 1.0, pxl, &xlo, nullptr));   // x_lo += a p
             TRY(v_axpby(c, ps, rs, -a, ps, q, 1.0, ps, &rs, &r2));          // r -= a q, ||r||^2
             k++; since_update++;
             rn = std::sqrt(r2);
             const bool update = (rn < c->delta * rmax) || (rn <= target) ||
                                 (c->max_update_interval > 0 && since_update >= c->max_update_interval);
+            double gam_new = 0;
             if (update) {
                 // reliable update: fold x_lo into x_hi and recompute the true residual in fp64
+                TRY(v_axpby(c, pxl, xlo, a, ps, p, 1.0, pxl, &xlo, nullptr));   // x_lo += a p
                 TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
                 TRY(v_zero(c, pxl, xlo));
                 TRY(op_Mpc(c, PDd, xhi, te, rhi));
@@ -610,11 +636,14 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
                 if (rn <= target) { converged = true; break; }
                 TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr));
                 rmax = rn;
+                TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));                 // g = Mpc^+ r, ||g||^2 fused
+                TRY(v_axpby(c, ps, p, 1.0, ps, g, gam_new / gam, ps, &p, nullptr));   // p = g + (gam'/gam) p
+            } else {
+                TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));
+                // x_lo += a p ; p = g + (gam'/gam) p in one pass over p
+                CUDA_OK(c, mdwf_launch_xpupdate(pxl, xlo, a, ps, p, gam_new / gam, g, c->L5, c->Vh, c->st));
+                c->launches += 1;
             }
-            TRY(op_Mpcdag(c, ps, rs, ts, g));                               // g = Mpc^+ r
-            double gam_new = 0;
-            TRY(v_norm2(c, ps, g, &gam_new));
-            TRY(v_axpby(c, ps, p, 1.0, ps, g, gam_new / gam, ps, &p, nullptr));   // p = g + (gam'/gam) p
             gam = gam_new;
         }
         if (!converged) {   // fold what we have
@@ -738,6 +767,14 @@ int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmu
     out4[3] = c->launches - l0;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
+    return MDWF_OK;
+}
+
+int mdwf_fma_rates(mdwf_ctx *c, double *tfma2)
+{
+    if (!c || !tfma2) return MDWF_EARG;
+    CUDA_OK(c, mdwf_measure_fma_rates(tfma2, c->st));
+    c->launches += 6;
     return MDWF_OK;
 }
 

@@ -50,6 +50,7 @@ struct HopArgs {
     double own_d, own_o;     // OWN = 2/3: adds (own_d + own_o Lambda[^dagger]) psi_own
     double post_d, post_o;   // POST = 2: applies (post_d + post_o Lambda^dagger) to coef_hop * hop
     double mf;
+    double *partial;         // v3 kernels: if non-null, ||out||^2 partial sums, one per block (fused norm, S7)
     const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
     // POST = 1 in the v3 kernels (hop3_kernels.cuh): coef_hop * B A^{-1} as a blocked recurrence
     int kver;                // host side: kernel family requested (2 or 3)
@@ -77,7 +78,12 @@ int mdwf_launch_axpby(Prec po, const SpinorBuf &out, double a, Prec px, const Sp
 // reductions on parity vectors: kind 0: ||x||^2, 1: Re<x,y>
 int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const SpinorBuf &y, int L5, int Vh,
                        double *partial, double *result_dev, cudaStream_t st);
+// fused CG update x += a p ; p = g + b p (x in precision px, p and g in precision pp)
+int mdwf_launch_xpupdate(Prec px, const SpinorBuf &x, double a, Prec pp, const SpinorBuf &p, double b, const SpinorBuf &g,
+                         int L5, int Vh, cudaStream_t st);
 int mdwf_reduce_max_blocks();
+// fixed-order sum of n partials into *result_dev (second pass of every reduction)
+int mdwf_launch_final_sum(const double *partial, int n, double *result_dev, cudaStream_t st);
 
 // flat-array BLAS-1 (mdwf_blas_* entry points)
 int mdwf_launch_flat_reduce(int kind, const void *x, const void *y, long long n, int real_bytes, double *partial,
@@ -103,3 +109,6 @@ int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed
 
 size_t mdwf_spinor_bytes(Prec p, int L5, int Vh);   // bytes of the chunk array
 size_t mdwf_gauge_bytes(Prec p, int Vh, int recon); // bytes of one parity's link array
+
+// fp32 FMA rates of this device (peak_kernels.cu): tfma[0] FFMA, tfma[1] packed FFMA2, in 1e12 FMA/s
+int mdwf_measure_fma_rates(double *tfma, cudaStream_t st);

@@ -21,6 +21,7 @@ def main():
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--reconstruct", default=None)
+    ap.add_argument("--fma-rates", action="store_true", help="also print the measured FFMA / FFMA2 rates")
     ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value")
     args = ap.parse_args()
     build.build()
@@ -34,6 +35,9 @@ def main():
     m.load_gauge(inputs.gauge_field(L, cfg["eps"], cfg["seed"], device="cuda"))
     torch.cuda.empty_cache()
     h = L[0] * L[1] * L[2] * L[3] // 2 * L5
+    if args.fma_rates:
+        r = m.fma_rates()
+        print(json.dumps({"ffma_tfma_per_s": r[0], "ffma2_tfma_per_s": r[1], "ffma_tflops": 2 * r[0], "ffma2_tflops": 2 * r[1]}), flush=True)
     F = m.flops_per_site()
     for prec in args.prec.split(","):
         rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[prec]
