@@ -266,12 +266,12 @@ def main():
                 "peak_source": peak_src, "traffic": None,
                 "algorithmic_bytes_per_launch": k1_bytes}
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
-    tf = os.path.join(ROOT, "profiles", "traffic.json")      # dram bytes per launch from the committed ncu capture
+    tf = os.path.join(ROOT, "profiles", "r01_traffic.csv")   # dram bytes per launch from the committed ncu capture
     if os.path.exists(tf):
-        try:
-            roofline["traffic"] = json.load(open(tf)).get("k1_%s_bytes_per_launch" % sloppy)
-        except Exception:
-            pass
+        for ln in open(tf).read().splitlines()[1:]:
+            k, _, v = ln.partition(",")
+            if k.strip() == "k1_%s" % sloppy:
+                roofline["traffic"] = float(v)
 
     ffma, ffma2 = m.fma_rates()
     # secondary view of the same kernel: fp32 lane operations it executes against the
