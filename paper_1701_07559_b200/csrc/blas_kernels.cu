@@ -30,7 +30,7 @@ __device__ __forceinline__ void block_partial(double v, double *partial)
     if (w == 0) {
         double t = (lane < RED_THREADS / 32) ? wsum[lane] : 0.0;
         t = warp_sum(t);
-        if (lane == 0) partial[blockIdx.x] = t;
+        if (lane == 0) partial[blockIdx.y * gridDim.x + blockIdx.x] = t;
     }
 }
 
@@ -64,34 +64,58 @@ static int red_blocks(long long work)
     return (int)b;
 }
 
+// grid of the parity-vector kernels: (nbx, L5) with nbx * L5 <= RED_MAX_BLOCKS partials
+static dim3 site_grid(int L5, int Vh)
+{
+    int nbx = (Vh + RED_THREADS - 1) / RED_THREADS;
+    const int cap = RED_MAX_BLOCKS / L5;
+    if (nbx > cap) nbx = cap;
+    if (nbx < 1) nbx = 1;
+    return dim3((unsigned)nbx, (unsigned)L5);
+}
+
 // ---- parity vectors: out = a x + b y  (+ ||out||^2) -------------------------------------------
+// arithmetic type of a BLAS kernel: fp64 as soon as one operand is stored in fp64, else fp32 (the result is
+// rounded to fp32 or 16 bits anyway); reductions always accumulate across sites in fp64
+template <class A, class B, class C> struct CompT { using T = float; };
+template <class B, class C> struct CompT<PD, B, C> { using T = double; };
+template <class C> struct CompT<PS, PD, C> { using T = double; };
+template <class C> struct CompT<PH, PD, C> { using T = double; };
+template <> struct CompT<PS, PS, PD> { using T = double; };
+template <> struct CompT<PS, PH, PD> { using T = double; };
+template <> struct CompT<PH, PS, PD> { using T = double; };
+template <> struct CompT<PH, PH, PD> { using T = double; };
+
 template <class PO, class PX, class PY, bool HASY, bool NORM>
 __global__ void __launch_bounds__(RED_THREADS)
 axpby_kernel(void *out, float *out_norm, double a, const void *x, const float *xn, double b, const void *y,
              const float *yn, int L5, long Vh, double *partial)
 {
     using RO = typename PO::R;
-    const long n5 = (long)L5 * Vh;
+    // grid = (blocks over the sites of one s-slice, L5): no integer division in the loop
+    const int s = blockIdx.y;
     double sum = 0.0;
-    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
-        const int s = (int)(idx / Vh);
-        const long cb = idx - (long)s * Vh;
+    for (long cb = (long)blockIdx.x * RED_THREADS + threadIdx.x; cb < Vh; cb += (long)gridDim.x * RED_THREADS) {
         typename PX::R vx[24];
         load_spinor<PX>(x, xn, L5, s, cb, vx);
+        using T = typename CompT<PO, PX, PY>::T;
+        const T ta = (T)a, tb = (T)b;
         RO r[24];
         if (HASY) {
             typename PY::R vy[24];
             load_spinor<PY>(y, yn, L5, s, cb, vy);
 #pragma unroll
-            for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k] + b * (double)vy[k]);
+            for (int k = 0; k < 24; k++) r[k] = (RO)(ta * (T)vx[k] + tb * (T)vy[k]);
         } else {
 #pragma unroll
-            for (int k = 0; k < 24; k++) r[k] = (RO)(a * (double)vx[k]);
+            for (int k = 0; k < 24; k++) r[k] = (RO)(ta * (T)vx[k]);
         }
         store_spinor<PO>(out, out_norm, L5, s, cb, r);
         if (NORM) {
+            T part = 0;
 #pragma unroll
-            for (int k = 0; k < 24; k++) sum += (double)r[k] * (double)r[k];
+            for (int k = 0; k < 24; k++) part += (T)r[k] * (T)r[k];
+            sum += (double)part;
         }
     }
     if (NORM) block_partial(sum, partial);
@@ -101,22 +125,24 @@ template <class PX, class PY, int KIND>
 __global__ void __launch_bounds__(RED_THREADS)
 reduce_kernel(const void *x, const float *xn, const void *y, const float *yn, int L5, long Vh, double *partial)
 {
-    const long n5 = (long)L5 * Vh;
+    // grid = (blocks over the sites of one s-slice, L5): no integer division in the loop
+    const int s = blockIdx.y;
     double sum = 0.0;
-    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
-        const int s = (int)(idx / Vh);
-        const long cb = idx - (long)s * Vh;
+    for (long cb = (long)blockIdx.x * RED_THREADS + threadIdx.x; cb < Vh; cb += (long)gridDim.x * RED_THREADS) {
         typename PX::R vx[24];
         load_spinor<PX>(x, xn, L5, s, cb, vx);
+        using T = typename CompT<PX, PY, PY>::T;
+        T part = 0;
         if (KIND == 0) {
 #pragma unroll
-            for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vx[k];
+            for (int k = 0; k < 24; k++) part += (T)vx[k] * (T)vx[k];
         } else {
             typename PY::R vy[24];
             load_spinor<PY>(y, yn, L5, s, cb, vy);
 #pragma unroll
-            for (int k = 0; k < 24; k++) sum += (double)vx[k] * (double)vy[k];
+            for (int k = 0; k < 24; k++) part += (T)vx[k] * (T)vy[k];
         }
+        sum += (double)part;
     }
     block_partial(sum, partial);
 }
@@ -125,7 +151,7 @@ template <class PO, class PX, class PY>
 static int axpby_xy(const SpinorBuf &out, double a, const SpinorBuf &x, double b, const SpinorBuf &y, int L5, int Vh,
                     double *partial, double *result, cudaStream_t st)
 {
-    const int nb = red_blocks((long long)L5 * Vh);
+    const dim3 nb = site_grid(L5, Vh);
     const bool hasy = (y.v != nullptr);
     const bool norm = (partial != nullptr);
 #define AX(HY, NM) axpby_kernel<PO, PX, PY, HY, NM><<<nb, RED_THREADS, 0, st>>>(out.v, out.norm, a, x.v, x.norm, b, y.v, y.norm, L5, Vh, partial)
@@ -134,7 +160,7 @@ static int axpby_xy(const SpinorBuf &out, double a, const SpinorBuf &x, double b
     else if (norm) AX(false, true);
     else AX(false, false);
 #undef AX
-    if (norm) final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, nb, result);
+    if (norm) final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, (int)(nb.x * nb.y), result);
     return (int)cudaGetLastError();
 }
 
@@ -173,12 +199,12 @@ template <class PX, class PY>
 static int reduce_xy(int kind, const SpinorBuf &x, const SpinorBuf &y, int L5, int Vh, double *partial,
                      double *result, cudaStream_t st)
 {
-    const int nb = red_blocks((long long)L5 * Vh);
+    const dim3 nb = site_grid(L5, Vh);
     if (kind == 0)
         reduce_kernel<PX, PY, 0><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, y.v, y.norm, L5, Vh, partial);
     else
         reduce_kernel<PX, PY, 1><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, y.v, y.norm, L5, Vh, partial);
-    final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, nb, result);
+    final_sum_kernel<<<1, RED_THREADS, 0, st>>>(partial, (int)(nb.x * nb.y), result);
     return (int)cudaGetLastError();
 }
 template <class PX>
@@ -206,19 +232,19 @@ template <class PX, class PP>
 __global__ void __launch_bounds__(RED_THREADS)
 xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, const void *g, const float *gn, int L5, long Vh)
 {
-    const long n5 = (long)L5 * Vh;
-    for (long idx = (long)blockIdx.x * RED_THREADS + threadIdx.x; idx < n5; idx += (long)gridDim.x * RED_THREADS) {
-        const int s = (int)(idx / Vh);
-        const long cb = idx - (long)s * Vh;
+    const int s = blockIdx.y;
+    for (long cb = (long)blockIdx.x * RED_THREADS + threadIdx.x; cb < Vh; cb += (long)gridDim.x * RED_THREADS) {
         typename PP::R vp[24], vg[24];
         typename PX::R vx[24];
         load_spinor<PP>(p, pn, L5, s, cb, vp);
         load_spinor<PP>(g, gn, L5, s, cb, vg);
         load_spinor<PX>(x, xn, L5, s, cb, vx);
+        using T = typename CompT<PX, PP, PP>::T;
+        const T ta = (T)a, tb = (T)b;
 #pragma unroll
         for (int k = 0; k < 24; k++) {
-            vx[k] = (typename PX::R)((double)vx[k] + a * (double)vp[k]);
-            vp[k] = (typename PP::R)((double)vg[k] + b * (double)vp[k]);
+            vx[k] = (typename PX::R)((T)vx[k] + ta * (T)vp[k]);
+            vp[k] = (typename PP::R)((T)vg[k] + tb * (T)vp[k]);
         }
         store_spinor<PX>(x, xn, L5, s, cb, vx);
         store_spinor<PP>(p, pn, L5, s, cb, vp);
@@ -228,7 +254,7 @@ template <class PX>
 static int xpupdate_p(Prec pp, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g, int L5, int Vh,
                       cudaStream_t st)
 {
-    const int nb = red_blocks((long long)L5 * Vh);
+    const dim3 nb = site_grid(L5, Vh);
 #define XP(PP) xpupdate_kernel<PX, PP><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, L5, Vh)
     switch (pp) {
     case PREC_D: XP(PD); break;

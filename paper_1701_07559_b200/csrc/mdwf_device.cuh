@@ -43,16 +43,25 @@ MDWF_DEV long sp_noff(int L5, long cb, int s) { return (((cb >> 5) * L5 + s) << 
 // ---- chunk <-> reals -------------------------------------------------------------------------
 MDWF_DEV void unpack(const double2 c, double *r, double) { r[0] = c.x; r[1] = c.y; }
 MDWF_DEV void unpack(const float4 c, float *r, float) { r[0] = c.x; r[1] = c.y; r[2] = c.z; r[3] = c.w; }
+// int16 -> fp32 on the integer and FMA pipes (the I2F conversion pipe runs at a quarter of their rate):
+// 0x4B400000 | (q ^ 0x8000) is the float 12582912 + 32768 + q; subtracting 12615680 is exact.
+MDWF_DEV float fixed_to_float(unsigned bits16)
+{
+    return __uint_as_float(0x4B400000u | (bits16 ^ 0x8000u)) - 12615680.0f;
+}
 MDWF_DEV void unpack(const short4 c, float *r, float sc)
 {
-    r[0] = sc * (float)c.x; r[1] = sc * (float)c.y; r[2] = sc * (float)c.z; r[3] = sc * (float)c.w;
+    r[0] = sc * fixed_to_float((unsigned short)c.x); r[1] = sc * fixed_to_float((unsigned short)c.y);
+    r[2] = sc * fixed_to_float((unsigned short)c.z); r[3] = sc * fixed_to_float((unsigned short)c.w);
 }
 MDWF_DEV double2 pack(const double *r, double, double2 *) { return make_double2(r[0], r[1]); }
 MDWF_DEV float4 pack(const float *r, float, float4 *) { return make_float4(r[0], r[1], r[2], r[3]); }
+// fp32 -> int16: the low 16 bits of fma(v, isc, 1.5 * 2^23) are round-to-nearest(v * isc) in two's complement
+MDWF_DEV short float_to_fixed(float v, float isc) { return (short)(__float_as_uint(fmaf(v, isc, 12582912.0f)) & 0xFFFFu); }
 MDWF_DEV short4 pack(const float *r, float isc, short4 *)
 {
-    return make_short4((short)__float2int_rn(r[0] * isc), (short)__float2int_rn(r[1] * isc),
-                       (short)__float2int_rn(r[2] * isc), (short)__float2int_rn(r[3] * isc));
+    return make_short4(float_to_fixed(r[0], isc), float_to_fixed(r[1], isc), float_to_fixed(r[2], isc),
+                       float_to_fixed(r[3], isc));
 }
 
 // Load NJ chunks starting at chunk pointer p (stride 32 chunks) into out[NJ*CH], scaled by sc (16-bit only).
@@ -107,7 +116,8 @@ MDWF_DEV void gunpack(const double2 c, double *r) { r[0] = c.x; r[1] = c.y; }
 MDWF_DEV void gunpack(const float2 c, float *r) { r[0] = c.x; r[1] = c.y; }
 MDWF_DEV void gunpack(const short2 c, float *r)
 {
-    r[0] = (float)c.x * (1.0f / MDWF_FIXED_MAX); r[1] = (float)c.y * (1.0f / MDWF_FIXED_MAX);
+    r[0] = fixed_to_float((unsigned short)c.x) * (1.0f / MDWF_FIXED_MAX);
+    r[1] = fixed_to_float((unsigned short)c.y) * (1.0f / MDWF_FIXED_MAX);
 }
 // U[2*(row*3+col)+ri]; with recon == 12 the third row is conj(row0 x row1).
 template <class P>
