@@ -80,37 +80,28 @@ MDWF_DEV void gget(const short2 q, float &re, float &im)
     re = v.x;
     im = v.y;
 }
-// stage one link (as stored: 6 or 9 complex chunks) from global into the block's shared-memory link table
-template <class P>
-MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, typename P::G *dst)
+// Build one link in pair form ONCE per block: load it as stored (6 or 9 complex chunks), rebuild row 2 for 12-real
+// storage, expand to (re,re) / (-im,im) (of U, or of U^dagger for a backward hop) and write the 9 float4
+// (R.x, R.y, I.x, I.y) of this lane to the block's shared-memory link table (element k at dst[32 k]).
+template <class P, bool DAGGER>
+MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, float4 *dst)
 {
     using G = typename P::G;
     const int NK = recon >> 1;
     const G *p = reinterpret_cast<const G *>(gbase) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
-    G tmp[9];
+    G raw[9];
 #pragma unroll
-    for (int k = 0; k < 6; k++) tmp[k] = __ldg(p + 32 * k);
+    for (int k = 0; k < 6; k++) raw[k] = __ldg(p + 32 * k);
     if (recon == 18) {
 #pragma unroll
-        for (int k = 6; k < 9; k++) tmp[k] = __ldg(p + 32 * k);
+        for (int k = 6; k < 9; k++) raw[k] = __ldg(p + 32 * k);
     }
-#pragma unroll
-    for (int k = 0; k < 6; k++) dst[32 * k] = tmp[k];
-    if (recon == 18) {
-#pragma unroll
-        for (int k = 6; k < 9; k++) dst[32 * k] = tmp[k];
-    }
-}
-// p = this lane's column of the shared-memory link table of one direction (element k at p[32 k])
-template <class P, bool DAGGER>
-MDWF_DEV void load_link3(const typename P::G *p, int recon, Link &L)
-{
     float ur[9], ui[9];
 #pragma unroll
-    for (int k = 0; k < 6; k++) gget(p[32 * k], ur[k], ui[k]);
+    for (int k = 0; k < 6; k++) gget(raw[k], ur[k], ui[k]);
     if (recon == 18) {
 #pragma unroll
-        for (int k = 6; k < 9; k++) gget(p[32 * k], ur[k], ui[k]);
+        for (int k = 6; k < 9; k++) gget(raw[k], ur[k], ui[k]);
     } else {
         // row2[c] = conj(row0[a] row1[b] - row0[b] row1[a]),  (a,b) = (c+1, c+2) mod 3
 #pragma unroll
@@ -128,14 +119,19 @@ MDWF_DEV void load_link3(const typename P::G *p, int recon, Link &L)
     for (int a = 0; a < 3; a++)
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            if (!DAGGER) {
-                L.R[a * 3 + c] = dup(ur[a * 3 + c]);
-                L.I[a * 3 + c] = mk(-ui[a * 3 + c], ui[a * 3 + c]);
-            } else {   // (U^dagger)_{ac} = conj(U_{ca})
-                L.R[a * 3 + c] = dup(ur[c * 3 + a]);
-                L.I[a * 3 + c] = mk(ui[c * 3 + a], -ui[c * 3 + a]);
-            }
+            if (!DAGGER) dst[32 * (a * 3 + c)] = make_float4(ur[a * 3 + c], ur[a * 3 + c], -ui[a * 3 + c], ui[a * 3 + c]);
+            else dst[32 * (a * 3 + c)] = make_float4(ur[c * 3 + a], ur[c * 3 + a], ui[c * 3 + a], -ui[c * 3 + a]);   // conj(U_ca)
         }
+}
+// p = this lane's column of the shared-memory link table of one direction
+MDWF_DEV void load_link3(const float4 *p, Link &L)
+{
+#pragma unroll
+    for (int k = 0; k < 9; k++) {
+        const float4 q = p[32 * k];
+        L.R[k] = mk(q.x, q.y);
+        L.I[k] = mk(q.z, q.w);
+    }
 }
 
 // chi[sp*3+a] = sum_c M[a][c] h[sp*3+c]: 6 FMUL2-started chains of 6 packed ops
@@ -225,13 +221,13 @@ MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
 // f * (slice s+1), wall factor -m_f at the wrap.  The window slides over the S slices (one half-spinor of
 // halo on each side), so only one full slice and two half slices are live at a time.
 template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR>
-MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const typename P::G *sl, long cb_nb, float bsign,
+MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float4 *sl, long cb_nb, float bsign,
                         c2 (*acc)[12], long cb_pf = -1)
 {
     using V = typename P::V;
     constexpr int SGN = (FWD ? 1 : -1) * (DAG ? -1 : 1);
     Link U;
-    load_link3<P, !FWD>(sl, a.recon, U);
+    load_link3(sl, U);
 
     const V *p0 = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, s0);
     const long n0 = sp_noff(L5, cb_nb, s0);
@@ -387,7 +383,7 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
     using V = typename P::V;
     extern __shared__ __align__(16) unsigned char smem_raw3[];
     c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
-    typename P::G *sL = reinterpret_cast<typename P::G *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
+    float4 *sL = reinterpret_cast<float4 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links in pair form
     const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
     long cb0 = (long)blockIdx.x * 32;
     if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
@@ -435,8 +431,8 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
 #pragma unroll
         for (int d = 0; d < 8; d++)
             if ((d % NSG) == sg) {
-                if ((d & 1) == 0) stage_link<P>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
-                else stage_link<P>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
+                if ((d & 1) == 0) stage_link<P, false>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
+                else stage_link<P, true>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
             }
     }
     __syncthreads();
@@ -560,7 +556,12 @@ static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
     constexpr int NSG = L5 / S;
     dim3 block(32, NSG);
     dim3 grid((unsigned)((a.Vh + 31) / 32));
-    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(typename P::G);
+    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float4);
+    if (smem > 32 * 1024) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
+        cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+    }
     hop3_kernel<P, DAG, PRE, POST, OWN, L5, S><<<grid, block, smem, st>>>(a);
     return (int)cudaGetLastError();
 }
