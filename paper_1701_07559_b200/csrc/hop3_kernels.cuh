@@ -67,10 +67,13 @@ template <> struct Ld<PH> {
     }
 };
 
-// ---- links in pair form -----------------------------------------------------------------------------
-// M = U (forward hop) or U^dagger (backward hop), entry (a,c):  R[a*3+c] = (re, re),  I[a*3+c] = (-im, im).
+// ---- links ---------------------------------------------------------------------------------------------
+// M = U (forward hop) or U^dagger (backward hop), entry (a,c) = re[a*3+c] + i im[a*3+c]: 18 scalar registers.
+// FFMA2 takes a scalar register broadcast to both lanes and a swapped (LO_HI) pair as free operand forms, so
+// chi_a = P + i Q with P = sum_c re (h_r,h_i), Q = sum_c im (h_r,h_i) needs no expanded copies of the link and no
+// register moves: chi = fma2((-1,1), (Q_i,Q_r), P).
 struct Link {
-    c2 R[9], I[9];
+    float re[9], im[9];
 };
 MDWF_DEV void gget(const float2 q, float &re, float &im) { re = q.x; im = q.y; }
 MDWF_DEV void gget(const short2 q, float &re, float &im)
@@ -80,11 +83,11 @@ MDWF_DEV void gget(const short2 q, float &re, float &im)
     re = v.x;
     im = v.y;
 }
-// Build one link in pair form ONCE per block: load it as stored (6 or 9 complex chunks), rebuild row 2 for 12-real
-// storage, expand to (re,re) / (-im,im) (of U, or of U^dagger for a backward hop) and write the 9 float4
-// (R.x, R.y, I.x, I.y) of this lane to the block's shared-memory link table (element k at dst[32 k]).
+// Build one link ONCE per block: load it as stored (6 or 9 complex chunks), rebuild row 2 for 12-real storage,
+// take the dagger for a backward hop, and write the 9 complex entries of this lane to the block's shared-memory
+// link table (element k at dst[32 k]).
 template <class P, bool DAGGER>
-MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, float4 *dst)
+MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, float2 *dst)
 {
     using G = typename P::G;
     const int NK = recon >> 1;
@@ -119,39 +122,37 @@ MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, float4 *
     for (int a = 0; a < 3; a++)
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            if (!DAGGER) dst[32 * (a * 3 + c)] = make_float4(ur[a * 3 + c], ur[a * 3 + c], -ui[a * 3 + c], ui[a * 3 + c]);
-            else dst[32 * (a * 3 + c)] = make_float4(ur[c * 3 + a], ur[c * 3 + a], ui[c * 3 + a], -ui[c * 3 + a]);   // conj(U_ca)
+            if (!DAGGER) dst[32 * (a * 3 + c)] = make_float2(ur[a * 3 + c], ui[a * 3 + c]);
+            else dst[32 * (a * 3 + c)] = make_float2(ur[c * 3 + a], -ui[c * 3 + a]);   // conj(U_ca)
         }
 }
 // p = this lane's column of the shared-memory link table of one direction
-MDWF_DEV void load_link3(const float4 *p, Link &L)
+MDWF_DEV void load_link3(const float2 *p, Link &L)
 {
 #pragma unroll
     for (int k = 0; k < 9; k++) {
-        const float4 q = p[32 * k];
-        L.R[k] = mk(q.x, q.y);
-        L.I[k] = mk(q.z, q.w);
+        const float2 q = p[32 * k];
+        L.re[k] = q.x;
+        L.im[k] = q.y;
     }
 }
 
-// chi[sp*3+a] = sum_c M[a][c] h[sp*3+c]: 6 FMUL2-started chains of 6 packed ops
+// chi[sp*3+a] = sum_c M[a][c] h[sp*3+c]: per output two chains of 3 packed operations and one combine
 MDWF_DEV void su3_mul3(const Link &L, const c2 *h, c2 *chi)
 {
-    c2 hs[6];
-#pragma unroll
-    for (int k = 0; k < 6; k++) hs[k] = swp(h[k]);
+    const c2 mp = mk(-1.f, 1.f);
 #pragma unroll
     for (int sp = 0; sp < 2; sp++)
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            c2 acc = mul2(L.R[a * 3], h[sp * 3]);
-            acc = fma2(L.I[a * 3], hs[sp * 3], acc);
+            c2 P = mul2(dup(L.re[a * 3]), h[sp * 3]);
+            c2 Q = mul2(dup(L.im[a * 3]), h[sp * 3]);
 #pragma unroll
             for (int c = 1; c < 3; c++) {
-                acc = fma2(L.R[a * 3 + c], h[sp * 3 + c], acc);
-                acc = fma2(L.I[a * 3 + c], hs[sp * 3 + c], acc);
+                P = fma2(dup(L.re[a * 3 + c]), h[sp * 3 + c], P);
+                Q = fma2(dup(L.im[a * 3 + c]), h[sp * 3 + c], Q);
             }
-            chi[sp * 3 + a] = acc;
+            chi[sp * 3 + a] = fma2(mp, mk(Q.y, Q.x), P);
         }
 }
 
@@ -221,7 +222,7 @@ MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
 // f * (slice s+1), wall factor -m_f at the wrap.  The window slides over the S slices (one half-spinor of
 // halo on each side), so only one full slice and two half slices are live at a time.
 template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR>
-MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float4 *sl, long cb_nb, float bsign,
+MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, long cb_nb, float bsign,
                         c2 (*acc)[12], long cb_pf = -1)
 {
     using V = typename P::V;
@@ -383,7 +384,7 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
     using V = typename P::V;
     extern __shared__ __align__(16) unsigned char smem_raw3[];
     c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
-    float4 *sL = reinterpret_cast<float4 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links in pair form
+    float2 *sL = reinterpret_cast<float2 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
     const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
     long cb0 = (long)blockIdx.x * 32;
     if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
@@ -556,7 +557,7 @@ static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
     constexpr int NSG = L5 / S;
     dim3 block(32, NSG);
     dim3 grid((unsigned)((a.Vh + 31) / 32));
-    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float4);
+    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float2);
     if (smem > 32 * 1024) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
         cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
