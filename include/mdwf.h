@@ -73,6 +73,10 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *                     conj(row0 x row1) in-kernel.  Takes effect at the next mdwf_load_gauge.  Default "18".
  *   "reliable_delta"  reliable-update threshold delta (default "0.1").
  *   "stream"          cudaStream_t as a decimal integer (default "0").
+ *   "kernels"         "v3" (default) | "v4" | "v2": kernel family for fp32 arithmetic. v3: hop3_kernels.cuh; v4: the same
+ *                     arithmetic with the neighbour groups staged in shared memory by bulk-asynchronous copies
+ *                     (Lx = 32, L5 in {8,12} only, else v3); v2: hop_kernels.cuh (always used for fp64 and other L5).
+ *   "sweep_mb"        L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
  *   "matpc"           "asym" only (the operator Chroma uses).
  */
 int mdwf_set_option(mdwf_ctx *ctx, const char *key, const char *value);

@@ -377,78 +377,12 @@ template <class P, int S> struct Hop3Cfg {
     static constexpr int WARPS = P::HALF ? MDWF_H3_WARPS_H : MDWF_H3_WARPS;
 };
 
-template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
-__global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S) > 0 ? Hop3Cfg<P, S>::WARPS / (L5 / S) : 1) hop3_kernel(const HopArgs a)
+// ---- epilogue shared by the v3 and v4 kernels: fifth-dimension POST step, own-site term, store, fused norm ----
+template <class P, int DAG, int POST, int OWN, int L5, int S>
+MDWF_DEV void epilogue3(const HopArgs &a, c2 (*acc)[12], c2 *sE, int lane, int sg, int s0, long cb, bool active)
 {
     constexpr int NSG = L5 / S;
     using V = typename P::V;
-    extern __shared__ __align__(16) unsigned char smem_raw3[];
-    c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
-    float2 *sL = reinterpret_cast<float2 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
-    const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
-    long cb0 = (long)blockIdx.x * 32;
-    if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
-        const int Lt = a.L[3];
-        const int per_chunk = a.sweep_nb * Lt;
-        const int c = blockIdx.x / per_chunk, r = blockIdx.x - c * per_chunk;
-        const int t = r / a.sweep_nb, q = r - t * a.sweep_nb;
-        cb0 = (long)t * ((long)a.Vh / Lt) + (long)c * a.sweep_chunk + (long)q * 32;
-    }
-    const long cb = cb0 + lane;
-    const bool active = cb < a.Vh;
-
-    c2 acc[S][12];
-#pragma unroll
-    for (int k = 0; k < S; k++)
-#pragma unroll
-        for (int q = 0; q < 12; q++) acc[k][q] = mk(0.f, 0.f);
-
-    // neighbour indices (inactive lanes of a ragged last block keep cb = 0 and load nothing)
-    const long cbs = active ? cb : 0;
-    const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
-    int r = (int)cbs;
-    const int xh = r % Lxh; r /= Lxh;
-    const int y = r % Ly;   r /= Ly;
-    const int z = r % Lz;
-    const int t = r / Lz;
-    const int xodd = (a.parity_out + y + z + t) & 1;
-    const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
-    long nb[8];
-    nb[0] = xodd ? (xh == Lxh - 1 ? cbs - (Lxh - 1) : cbs + 1) : cbs;
-    nb[1] = xodd ? cbs : (xh == 0 ? cbs + (Lxh - 1) : cbs - 1);
-    nb[2] = (y == Ly - 1) ? cbs - (Ly - 1) * sy : cbs + sy;
-    nb[3] = (y == 0) ? cbs + (Ly - 1) * sy : cbs - sy;
-    nb[4] = (z == Lz - 1) ? cbs - (Lz - 1) * sz : cbs + sz;
-    nb[5] = (z == 0) ? cbs + (Lz - 1) * sz : cbs - sz;
-    nb[6] = (t == Lt - 1) ? cbs - (Lt - 1) * st : cbs + st;
-    nb[7] = (t == 0) ? cbs + (Lt - 1) * st : cbs - st;
-    const float btp = (t == Lt - 1) ? -1.f : 1.f;               // antiperiodic in t
-    const float btm = (t == 0) ? -1.f : 1.f;
-
-    // stage the 8 links of the block's 32 sites in shared memory once: direction d = 2 mu + (0 fwd, 1 bwd) is
-    // fetched by warp d mod NSG; the NSG warps of a site then read them from there (no per-direction global
-    // latency on the critical path, 1/NSG of the global link loads)
-    if (active) {
-#pragma unroll
-        for (int d = 0; d < 8; d++)
-            if ((d % NSG) == sg) {
-                if ((d & 1) == 0) stage_link<P, false>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
-                else stage_link<P, true>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
-            }
-    }
-    __syncthreads();
-
-    if (active) {
-        hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, nb[0], 1.f, acc);
-        hop_dir3<P, 0, false, DAG, PRE, S, false>(a, L5, s0, sL + 1 * 288 + lane, nb[1], 1.f, acc);
-        hop_dir3<P, 1, true, DAG, PRE, S, false>(a, L5, s0, sL + 2 * 288 + lane, nb[2], 1.f, acc);
-        hop_dir3<P, 1, false, DAG, PRE, S, false>(a, L5, s0, sL + 3 * 288 + lane, nb[3], 1.f, acc);
-        hop_dir3<P, 2, true, DAG, PRE, S, false>(a, L5, s0, sL + 4 * 288 + lane, nb[4], 1.f, acc);
-        hop_dir3<P, 2, false, DAG, PRE, S, false>(a, L5, s0, sL + 5 * 288 + lane, nb[5], 1.f, acc);
-        hop_dir3<P, 3, true, DAG, PRE, S, true>(a, L5, s0, sL + 6 * 288 + lane, nb[6], btp, acc);
-        hop_dir3<P, 3, false, DAG, PRE, S, true>(a, L5, s0, sL + 7 * 288 + lane, nb[7], btm, acc);
-    }
-
     if (POST == 1) {
         // coef_hop * (B A^{-1}) acc per chirality (DAG: the transposed pattern) by blocked recurrence
         const c2 nk = dup(a.r_nk);
@@ -548,6 +482,81 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
             a.partial[blockIdx.x] = t;
         }
     }
+}
+
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+__global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S) > 0 ? Hop3Cfg<P, S>::WARPS / (L5 / S) : 1) hop3_kernel(const HopArgs a)
+{
+    constexpr int NSG = L5 / S;
+    using V = typename P::V;
+    extern __shared__ __align__(16) unsigned char smem_raw3[];
+    c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
+    float2 *sL = reinterpret_cast<float2 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
+    const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
+    long cb0 = (long)blockIdx.x * 32;
+    if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
+        const int Lt = a.L[3];
+        const int per_chunk = a.sweep_nb * Lt;
+        const int c = blockIdx.x / per_chunk, r = blockIdx.x - c * per_chunk;
+        const int t = r / a.sweep_nb, q = r - t * a.sweep_nb;
+        cb0 = (long)t * ((long)a.Vh / Lt) + (long)c * a.sweep_chunk + (long)q * 32;
+    }
+    const long cb = cb0 + lane;
+    const bool active = cb < a.Vh;
+
+    c2 acc[S][12];
+#pragma unroll
+    for (int k = 0; k < S; k++)
+#pragma unroll
+        for (int q = 0; q < 12; q++) acc[k][q] = mk(0.f, 0.f);
+
+    // neighbour indices (inactive lanes of a ragged last block keep cb = 0 and load nothing)
+    const long cbs = active ? cb : 0;
+    const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
+    int r = (int)cbs;
+    const int xh = r % Lxh; r /= Lxh;
+    const int y = r % Ly;   r /= Ly;
+    const int z = r % Lz;
+    const int t = r / Lz;
+    const int xodd = (a.parity_out + y + z + t) & 1;
+    const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
+    long nb[8];
+    nb[0] = xodd ? (xh == Lxh - 1 ? cbs - (Lxh - 1) : cbs + 1) : cbs;
+    nb[1] = xodd ? cbs : (xh == 0 ? cbs + (Lxh - 1) : cbs - 1);
+    nb[2] = (y == Ly - 1) ? cbs - (Ly - 1) * sy : cbs + sy;
+    nb[3] = (y == 0) ? cbs + (Ly - 1) * sy : cbs - sy;
+    nb[4] = (z == Lz - 1) ? cbs - (Lz - 1) * sz : cbs + sz;
+    nb[5] = (z == 0) ? cbs + (Lz - 1) * sz : cbs - sz;
+    nb[6] = (t == Lt - 1) ? cbs - (Lt - 1) * st : cbs + st;
+    nb[7] = (t == 0) ? cbs + (Lt - 1) * st : cbs - st;
+    const float btp = (t == Lt - 1) ? -1.f : 1.f;               // antiperiodic in t
+    const float btm = (t == 0) ? -1.f : 1.f;
+
+    // stage the 8 links of the block's 32 sites in shared memory once: direction d = 2 mu + (0 fwd, 1 bwd) is
+    // fetched by warp d mod NSG; the NSG warps of a site then read them from there (no per-direction global
+    // latency on the critical path, 1/NSG of the global link loads)
+    if (active) {
+#pragma unroll
+        for (int d = 0; d < 8; d++)
+            if ((d % NSG) == sg) {
+                if ((d & 1) == 0) stage_link<P, false>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
+                else stage_link<P, true>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
+            }
+    }
+    __syncthreads();
+
+    if (active) {
+        hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, nb[0], 1.f, acc);
+        hop_dir3<P, 0, false, DAG, PRE, S, false>(a, L5, s0, sL + 1 * 288 + lane, nb[1], 1.f, acc);
+        hop_dir3<P, 1, true, DAG, PRE, S, false>(a, L5, s0, sL + 2 * 288 + lane, nb[2], 1.f, acc);
+        hop_dir3<P, 1, false, DAG, PRE, S, false>(a, L5, s0, sL + 3 * 288 + lane, nb[3], 1.f, acc);
+        hop_dir3<P, 2, true, DAG, PRE, S, false>(a, L5, s0, sL + 4 * 288 + lane, nb[4], 1.f, acc);
+        hop_dir3<P, 2, false, DAG, PRE, S, false>(a, L5, s0, sL + 5 * 288 + lane, nb[5], 1.f, acc);
+        hop_dir3<P, 3, true, DAG, PRE, S, true>(a, L5, s0, sL + 6 * 288 + lane, nb[6], btp, acc);
+        hop_dir3<P, 3, false, DAG, PRE, S, true>(a, L5, s0, sL + 7 * 288 + lane, nb[7], btm, acc);
+    }
+
+    epilogue3<P, DAG, POST, OWN, L5, S>(a, acc, sE, lane, sg, s0, cb, active);
 }
 
 // ---- launchers ----------------------------------------------------------------------------------

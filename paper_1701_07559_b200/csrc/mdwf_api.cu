@@ -15,6 +15,8 @@
 int mdwf_launch_hop_D(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop4_S(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop4_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
@@ -23,6 +25,11 @@ int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const v
 
 int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
 {
+    if (a.kver >= 4 && p != PREC_D) {        // v4 family (staged neighbours); -1 = not covered, fall back to v3
+        const int rc = (p == PREC_S) ? mdwf_launch_hop4_S(dag, pre, post, own, a, st)
+                                     : mdwf_launch_hop4_H(dag, pre, post, own, a, st);
+        if (rc != -1) return rc;
+    }
     if (a.kver >= 3 && p != PREC_D) {        // v3 family (fp32 arithmetic); -1 = not covered, fall back to v2
         const int rc = (p == PREC_S) ? mdwf_launch_hop3_S(dag, pre, post, own, a, st)
                                      : mdwf_launch_hop3_H(dag, pre, post, own, a, st);
@@ -449,8 +456,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
     } else if (k == "kernels") {
-        if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
-        else { c->err = "kernels must be v2|v3"; return MDWF_EARG; }
+        if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
+        else { c->err = "kernels must be v2|v3|v4"; return MDWF_EARG; }
     } else if (k == "sweep_mb") {
         c->sweep_mb = atoi(value);
     } else if (k == "stream") {

@@ -49,13 +49,15 @@ def test_mpc_sampled_sites_at_config4():
     sites = sample_sites(orc, 48, 7)
     cbs = torch.from_numpy(sites // 2).cuda()
     ref = {binding.OP_MPC: orc.Mpc_at_sites(v_o, sites), binding.OP_MPCDAG: orc.Mpc_at_sites(v_o, sites, dagger=True)}
-    for prec in ("fp64", "fp32", "half"):
+    # v3 = default kernels (hop3_kernels.cuh); v4 = neighbours staged by bulk-asynchronous copies (hop4_kernels.cuh)
+    for kern, prec in (("v3", "fp64"), ("v3", "fp32"), ("v3", "half"), ("v4", "fp32"), ("v4", "half")):
+        m.set_option("kernels", kern)
         m.set_option("apply_precision", prec)
         x = bo_dev if prec == "fp64" else bo_dev.to(torch.complex64)
         for op, r in ref.items():
             got = m.apply(op, x)[:, cbs].cpu().numpy().astype(np.complex128)
             assert got.shape == r.shape
-            assert rel(got, r) < TOL[prec], (prec, op, rel(got, r))
+            assert rel(got, r) < TOL[prec], (kern, prec, op, rel(got, r))
             # every sampled site individually (a wrong wrap or sign shows up as an O(1) error on one site)
             per_site = np.linalg.norm((got - r).reshape(L5, len(sites), -1), axis=(0, 2)) / \
                 np.linalg.norm(r.reshape(L5, len(sites), -1), axis=(0, 2))
