@@ -18,6 +18,7 @@ CASES = {
     "l5_12": ((6, 4, 2, 8), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 3),         # several blocks, config-4 parameters
     "l5_16": ((2, 2, 4, 4), 16, 1.3, 1.75, 0.75, 0.00712, 0.2, 5),     # a15m220 row of Table II
     "l5_24": ((2, 2, 2, 4), 24, 1.3, 2.25, 1.25, 0.00216, 0.2, 6),     # a15m130 row of Table II (generic path)
+    "lx32": ((32, 4, 2, 4), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 7),         # Lx = 32: the geometry the v4 (staged) kernels cover
 }
 TOL = {"fp64": 1e-12, "fp32": 1e-5, "half": 2e-3}
 
@@ -60,6 +61,26 @@ def test_operator_parity(name, prec, recon):
     for op, r in ((binding.OP_D, orc.D(b)), (binding.OP_DDAG, orc.Ddag(b))):
         got = m.apply(op, xf).cpu().numpy().astype(np.complex128)
         assert rel(got, r) < TOL[prec], (name, prec, recon, op)
+    m.close()
+
+
+@pytest.mark.parametrize("name", ["lx32", "l5_12"])       # l5_12: v4 is not applicable and must fall back to v3
+@pytest.mark.parametrize("prec", ["fp32", "half"])
+def test_operator_parity_v4_kernels(name, prec):
+    """the bulk-copy staged kernel family (option kernels=v4), incl. the y wrap-around at Ly = 4"""
+    from paper_1701_07559_b200 import binding
+    orc, m, b = setup(name, "12")
+    m.set_option("kernels", "v4")
+    m.set_option("apply_precision", prec)
+    bo_full = orc.parity_part(b, 1)
+    x = to_dev(orc.pack_parity(b, 1), prec)
+    for op, r in ((binding.OP_MPC, orc.Mpc(bo_full)), (binding.OP_MPCDAG, orc.Mpcdag(bo_full))):
+        got = m.apply(op, x).cpu().numpy().astype(np.complex128)
+        assert rel(got, orc.pack_parity(r, 1)) < TOL[prec], (name, prec, op)
+    xf = to_dev(b, prec)
+    for op, r in ((binding.OP_D, orc.D(b)), (binding.OP_DDAG, orc.Ddag(b))):
+        got = m.apply(op, xf).cpu().numpy().astype(np.complex128)
+        assert rel(got, r) < TOL[prec], (name, prec, op)
     m.close()
 
 
