@@ -5,9 +5,10 @@
 // s-slices; block = 32 sites x L5/S warps), rebuilt around three B200 facts measured in profiles/:
 //   1. sm_100a issues a 3-register FFMA at half rate; the packed FFMA2 (fma.rn.f32x2) carries two FMAs per
 //      lane and reaches 65 TFLOP/s against 40 for FFMA.  A complex number is one float2 register pair and
-//      every arithmetic step below is a packed f32x2 instruction: SU(3) x half-spinor is
-//      chi_a = sum_c (ur,ur)*(hr,hi) + (-ui,ui)*(hi,hr); the links are expanded once per direction into those
-//      two pair forms and reused for the S slices and both spin components.
+//      every arithmetic step below is a packed f32x2 instruction.  FFMA2 takes a scalar register broadcast to
+//      both lanes and a swapped pair as free operand forms, so SU(3) x half-spinor is chi_a = P + iQ with
+//      P = sum_c ur (hr,hi), Q = sum_c ui (hr,hi): the link stays 18 scalars, reused for the S slices and both
+//      spin components, and multiplication by +-i costs nothing.
 //   2. The dense L5 x L5 matrix B A^{-1} (S3 of the hot path) is semiseparable: A = alpha (1 + kappa T) with T
 //      the cyclic shift carrying -m_f at the wall, so A^{-1} is a first-order recurrence plus a rank-one wall
 //      term.  Each thread runs the recurrence over its own S slices in registers, the warps of a block
@@ -15,7 +16,10 @@
 //          t_s = (b5 z_s + c5 z_{s-1}) / alpha + qW_s W,    z_s = x_s - kappa z_{s-1},  W = z_{L5-1}
 //      replaces 2 L5 FMAs per real by about 6 (DESIGN.md section 5 derives it; the fp64 path and any L5 outside
 //      {8,12,16} keep the dense table of hop_kernels.cuh).
-//   3. No register spills: the s-window of the B-on-load stencil slides slice by slice.
+//   3. The first stall of every direction used to be the link load: the 8 links of the block's 32 sites are built
+//      ONCE per block in shared memory (12-real reconstruction and the dagger of backward hops included) and
+//      read back with 9 LDS.64 per direction.  No register spills: the s-window of the B-on-load stencil slides
+//      slice by slice.
 #pragma once
 #include "mdwf_device.cuh"
 #include "mdwf_internal.h"
