@@ -49,15 +49,15 @@ template <> struct Ld<PS> {
         }
     }
 };
-// 16-bit fixed point -> fp32 without the conversion pipe: 0x4B400000 | (q ^ 0x8000) is the float 12582912 + 32768 + q,
-// so value = (that - 12615680) * scale, both steps exact up to the one rounding of the product: one LOP3 per
-// word, one PRMT per value, one FADD2 + one FMUL2 per complex.
-MDWF_DEV c2 cvt_pair(unsigned w, c2 sc)      // w = two int16 (low half = first)
+// 16-bit fixed point -> fp32 without the conversion pipe.  The 16 bits are stored offset-binary (u = q + 32768), so
+// 0x4B400000 | u is the float 12582912 + 32768 + q and value = (that - 12615680) * scale, both steps exact up to the
+// one rounding of the product: one PRMT per value, one FADD2 (+ one FMUL2) per complex.
+MDWF_DEV c2 cvt_raw(unsigned w)                // w = two 16-bit values (low half = first) -> the two integers as floats
 {
-    const unsigned x = w ^ 0x80008000u;
-    const c2 f = mk(__uint_as_float(__byte_perm(x, 0x4B400000u, 0x7610)), __uint_as_float(__byte_perm(x, 0x4B400000u, 0x7632)));
-    return mul2(add2(f, dup(-12615680.0f)), sc);
+    const c2 f = mk(__uint_as_float(__byte_perm(w, 0x4B400000u, 0x7610)), __uint_as_float(__byte_perm(w, 0x4B400000u, 0x7632)));
+    return add2(f, dup(-12615680.0f));
 }
+MDWF_DEV c2 cvt_pair(unsigned w, c2 sc) { return mul2(cvt_raw(w), sc); }
 template <> struct Ld<PH> {
     template <int NC> static MDWF_DEV void chunks(const short4 *p, float sc, c2 *v)
     {
@@ -67,6 +67,17 @@ template <> struct Ld<PH> {
             const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p + 32 * j));
             v[2 * j] = cvt_pair(q.x, s2);
             v[2 * j + 1] = cvt_pair(q.y, s2);
+        }
+    }
+    // the stored integers as floats, unscaled: the hop is linear, so the scale of the slice is applied once, in the
+    // reconstruction FMAs (saves one FMUL2 per complex on every neighbour load without B-on-load)
+    template <int NC> static MDWF_DEV void raw(const short4 *p, c2 *v)
+    {
+#pragma unroll
+        for (int j = 0; j < NC / 2; j++) {
+            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p + 32 * j));
+            v[2 * j] = cvt_raw(q.x);
+            v[2 * j + 1] = cvt_raw(q.y);
         }
     }
 };
@@ -242,10 +253,18 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, long 
 #pragma unroll
         for (int k = 0; k < S; k++) {
             c2 v[12], h[6], chi[6];
-            Ld<P>::template chunks<12>(p0 + k * SL, load_scale<P>(a.in_norm, n0 + 32 * k), v);
-            project3<MU, SGN>(v, h);
-            su3_mul3(U, h, chi);
-            recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
+            if constexpr (P::HALF) {
+                const float sck = load_scale<P>(a.in_norm, n0 + 32 * k);
+                Ld<P>::template raw<12>(p0 + k * SL, v);
+                project3<MU, SGN>(v, h);
+                su3_mul3(U, h, chi);
+                recon3<MU, SGN, true>(chi, TDIR ? bsign * sck : sck, acc[k]);
+            } else {
+                Ld<P>::template chunks<12>(p0 + k * SL, load_scale<P>(a.in_norm, n0 + 32 * k), v);
+                project3<MU, SGN>(v, h);
+                su3_mul3(U, h, chi);
+                recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
+            }
         }
     } else {
         const float f = (float)(a.pre_o / a.pre_d), fw = (float)(-a.mf * a.pre_o / a.pre_d);
@@ -306,10 +325,10 @@ template <> MDWF_DEV float store3<PH>(void *base, float *norm, int L5, int s, lo
 #pragma unroll
     for (int q = 0; q < 12; q++) m = fmaxf(m, fmaxf(fabsf(o[q].x), fabsf(o[q].y)));
     norm[sp_noff(L5, cb, s)] = m;
-    // fp32 -> 16-bit fixed point by the magic-number add: the low 16 bits of fma(v, isc, 1.5 * 2^23) are round(v isc)
-    const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f), magic = dup(12582912.0f);
+    // fp32 -> 16-bit offset binary by the magic-number add: the low 16 bits of fma(v, isc, 1.5 * 2^23 + 2^15) are round(v isc) + 2^15
+    const c2 isc = dup(m > 0.f ? MDWF_FIXED_MAX / m : 0.f), magic = dup(12615680.0f);
     uint2 *pw = reinterpret_cast<uint2 *>(p);
-    const c2 nmagic = dup(-12582912.0f);
+    const c2 nmagic = dup(-12615680.0f);
     c2 n2 = mk(0.f, 0.f);
 #pragma unroll
     for (int j = 0; j < 6; j++) {

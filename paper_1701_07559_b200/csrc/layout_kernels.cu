@@ -66,7 +66,9 @@ MDWF_DEV double2 gpack(double re, double im, double2 *) { return make_double2(re
 MDWF_DEV float2 gpack(double re, double im, float2 *) { return make_float2((float)re, (float)im); }
 MDWF_DEV short2 gpack(double re, double im, short2 *)
 {
-    return make_short2((short)__double2int_rn(re * (double)MDWF_FIXED_MAX), (short)__double2int_rn(im * (double)MDWF_FIXED_MAX));
+    // offset binary, like the spinors (mdwf_device.cuh)
+    return make_short2((short)(unsigned short)(__double2int_rn(re * (double)MDWF_FIXED_MAX) + 32768),
+                       (short)(unsigned short)(__double2int_rn(im * (double)MDWF_FIXED_MAX) + 32768));
 }
 
 template <class P, class T>

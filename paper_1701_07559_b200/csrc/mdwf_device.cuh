@@ -28,7 +28,7 @@ struct PS {   // fp32 storage and arithmetic
     static constexpr int CH = 4;
     static constexpr bool HALF = false;
 };
-struct PH {   // 16-bit fixed-point storage (+ one fp32 scale per 5D site), fp32 arithmetic
+struct PH {   // 16-bit fixed-point storage, offset binary (+ one fp32 scale per 5D site), fp32 arithmetic
     using R = float; using V = short4; using G = short2;
     static constexpr int NV = 6;
     static constexpr int CH = 4;
@@ -44,10 +44,11 @@ MDWF_DEV long sp_noff(int L5, long cb, int s) { return (((cb >> 5) * L5 + s) << 
 MDWF_DEV void unpack(const double2 c, double *r, double) { r[0] = c.x; r[1] = c.y; }
 MDWF_DEV void unpack(const float4 c, float *r, float) { r[0] = c.x; r[1] = c.y; r[2] = c.z; r[3] = c.w; }
 // int16 -> fp32 on the integer and FMA pipes (the I2F conversion pipe runs at a quarter of their rate):
-// 0x4B400000 | (q ^ 0x8000) is the float 12582912 + 32768 + q; subtracting 12615680 is exact.
+// the 16 bits are stored offset-binary (u = q + 32768), so 0x4B400000 | u is the float 12582912 + 32768 + q;
+// subtracting 12615680 is exact.
 MDWF_DEV float fixed_to_float(unsigned bits16)
 {
-    return __uint_as_float(0x4B400000u | (bits16 ^ 0x8000u)) - 12615680.0f;
+    return __uint_as_float(0x4B400000u | bits16) - 12615680.0f;
 }
 MDWF_DEV void unpack(const short4 c, float *r, float sc)
 {
@@ -56,8 +57,8 @@ MDWF_DEV void unpack(const short4 c, float *r, float sc)
 }
 MDWF_DEV double2 pack(const double *r, double, double2 *) { return make_double2(r[0], r[1]); }
 MDWF_DEV float4 pack(const float *r, float, float4 *) { return make_float4(r[0], r[1], r[2], r[3]); }
-// fp32 -> int16: the low 16 bits of fma(v, isc, 1.5 * 2^23) are round-to-nearest(v * isc) in two's complement
-MDWF_DEV short float_to_fixed(float v, float isc) { return (short)(__float_as_uint(fmaf(v, isc, 12582912.0f)) & 0xFFFFu); }
+// fp32 -> 16 bits: the low 16 bits of fma(v, isc, 1.5 * 2^23 + 32768) are round-to-nearest(v * isc) + 32768
+MDWF_DEV short float_to_fixed(float v, float isc) { return (short)(__float_as_uint(fmaf(v, isc, 12615680.0f)) & 0xFFFFu); }
 MDWF_DEV short4 pack(const float *r, float isc, short4 *)
 {
     return make_short4(float_to_fixed(r[0], isc), float_to_fixed(r[1], isc), float_to_fixed(r[2], isc),
