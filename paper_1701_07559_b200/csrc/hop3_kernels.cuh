@@ -619,6 +619,7 @@ template <class P>
 static int launch_hop3_prec(int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
 {
     if (!dag && pre == 1 && post == 1 && own == 0) return launch_hop3_l5<P, 0, 1, 1, 0>(a, st);   // K1
+    if (!dag && pre == 0 && post == 1 && own == 0) return launch_hop3_l5<P, 0, 0, 1, 0>(a, st);   // K1 reading a precomputed B psi
     if (!dag && pre == 0 && post == 0 && own == 2) return launch_hop3_l5<P, 0, 0, 0, 2>(a, st);   // K2
     if (!dag && pre == 1 && post == 0 && own == 2) return launch_hop3_l5<P, 0, 1, 0, 2>(a, st);   // D
     if (!dag && pre == 1 && post == 0 && own == 1) return launch_hop3_l5<P, 0, 1, 0, 1>(a, st);   // Schur prep/recon

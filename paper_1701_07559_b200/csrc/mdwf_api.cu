@@ -4,6 +4,7 @@
 #include "../../include/mdwf.h"
 #include "mdwf_internal.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -64,6 +65,7 @@ struct mdwf_ctx {
     int apply_prec = -1;     // -1 auto
     double delta = 0.1;
     int max_update_interval = 0;
+    int use_bp = 1;          // 16-bit Krylov vectors: let the CG update write B p for K1 (option "bp_stream")
     int kver = 3;            // kernel family for fp32 arithmetic: 3 = hop3_kernels.cuh, 2 = hop_kernels.cuh
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
@@ -287,6 +289,13 @@ static int op_Mpc_k1(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &
     k1.coef_hop = c->b5; k1.pre_d = c->b5; k1.pre_o = c->c5; k1.dense = dense_ptr(c, p, DENSE_BAINV);   // b5 of B-on-load folded in
     return run_hop(c, p, 0, 1, 1, 0, k1);
 }
+// K1 of Mpc from a precomputed B in_o (written by the fused CG update for 16-bit vectors): t_e = (B A^{-1}) H_eo (B in)_o
+static int op_Mpc_k1_from_B(mdwf_ctx *c, Prec p, const SpinorBuf &Bin, const SpinorBuf &tmp)
+{
+    HopArgs k1 = base_args(c, p, 0, Bin, nullptr, tmp);
+    k1.coef_hop = 1.0; k1.dense = dense_ptr(c, p, DENSE_BAINV);
+    return run_hop(c, p, 0, 0, 1, 0, k1);
+}
 // the v3 kernels can emit ||out||^2 partials from their epilogue (fused norm)
 static bool fused_norm_available(const mdwf_ctx *c, Prec p)
 {
@@ -458,6 +467,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "kernels") {
         if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
         else { c->err = "kernels must be v2|v3|v4"; return MDWF_EARG; }
+    } else if (k == "bp_stream") {
+        c->use_bp = atoi(value);
     } else if (k == "sweep_mb") {
         c->sweep_mb = atoi(value);
     } else if (k == "stream") {
@@ -583,6 +594,10 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     TRY(get_spinor(c, "sv.q", ps, &q));
     TRY(get_spinor(c, "sv.ts", ps, &ts));
     TRY(get_spinor(c, "sv.xlo", pxl, &xlo));
+    // 16-bit Krylov vectors: the CG update also writes B p, and p is double-buffered
+    const bool use_bp = (ps == PREC_H) && fused_norm_available(c, ps) && c->use_bp;
+    SpinorBuf p2, bpv;
+    if (use_bp) { TRY(get_spinor(c, "sv.p2", ps, &p2)); TRY(get_spinor(c, "sv.bp", ps, &bpv)); }
 
     c->iterations = 0; c->reliable_updates = 0; c->op_applications = 0; c->sloppy_applications = 0;
 
@@ -618,10 +633,36 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
         TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr)); // r_s = convert(r_hi)
         TRY(op_Mpcdag(c, ps, rs, ts, g));                                   // g = Mpc^+ r
         double gam = 0;
-        TRY(v_axpby(c, ps, p, 1.0, ps, g, 0.0, ps, nullptr, &gam));         // p = g, gam = ||g||^2
+        SpinorBuf pc = p, pn = p2;                                          // current / next direction vector (use_bp)
+        // fused update; with use_bp it also writes B p_new and flips the double buffer of p
+        auto cg_update = [&](double ax, double bx) -> int {
+            if (use_bp) {
+                CUDA_OK(c, mdwf_launch_xpupdate_b(pxl, xlo, ax, pc, bx, g, pn, bpv, c->b5, c->c5, c->mf, c->L5, c->Vh, c->st));
+                std::swap(pc, pn);
+            } else {
+                CUDA_OK(c, mdwf_launch_xpupdate(pxl, xlo, ax, ps, pc, bx, g, c->L5, c->Vh, c->st));
+            }
+            c->launches += 1;
+            return MDWF_OK;
+        };
+        auto apply_Mpc = [&](double *qq) -> int {                           // q = Mpc p, ||q||^2 from the K2 epilogue
+            if (!use_bp) return op_Mpc(c, ps, pc, ts, q, qq);
+            TRY(op_Mpc_k1_from_B(c, ps, bpv, ts));
+            TRY(op_Mpc_k2(c, ps, pc, ts, q, qq));
+            c->op_applications += 1;
+            c->sloppy_applications += 1;
+            return MDWF_OK;
+        };
+        if (use_bp) {
+            TRY(v_norm2(c, ps, g, &gam));
+            TRY(v_zero(c, ps, pc));
+            TRY(cg_update(0.0, 0.0));                                       // p = g, B p
+        } else {
+            TRY(v_axpby(c, ps, pc, 1.0, ps, g, 0.0, ps, nullptr, &gam));    // p = g, gam = ||g||^2
+        }
         while (k < maxiter && !converged) {
             double qq = 0;
-            TRY(op_Mpc(c, ps, p, ts, q, &qq));                              // q = Mpc p, ||q||^2 from the K2 epilogue
+            TRY(apply_Mpc(&qq));
             if (!(qq > 0.0) || !(gam > 0.0)) break;
             const double a = gam / qq;
             TRY(v_axpby(c, ps, rs, -a, ps, q, 1.0, ps, &rs, &r2));          // r -= a q, ||r||^2
@@ -632,7 +673,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
             double gam_new = 0;
             if (update) {
                 // reliable update: fold x_lo into x_hi and recompute the true residual in fp64
-                TRY(v_axpby(c, pxl, xlo, a, ps, p, 1.0, pxl, &xlo, nullptr));   // x_lo += a p
+                TRY(v_axpby(c, pxl, xlo, a, ps, pc, 1.0, pxl, &xlo, nullptr));  // x_lo += a p
                 TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
                 TRY(v_zero(c, pxl, xlo));
                 TRY(op_Mpc(c, PDd, xhi, te, rhi));
@@ -644,12 +685,10 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
                 TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr));
                 rmax = rn;
                 TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));                 // g = Mpc^+ r, ||g||^2 fused
-                TRY(v_axpby(c, ps, p, 1.0, ps, g, gam_new / gam, ps, &p, nullptr));   // p = g + (gam'/gam) p
+                TRY(cg_update(0.0, gam_new / gam));                         // p = g + (gam'/gam) p   (x_lo is zero)
             } else {
                 TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));
-                // x_lo += a p ; p = g + (gam'/gam) p in one pass over p
-                CUDA_OK(c, mdwf_launch_xpupdate(pxl, xlo, a, ps, p, gam_new / gam, g, c->L5, c->Vh, c->st));
-                c->launches += 1;
+                TRY(cg_update(a, gam_new / gam));                           // x_lo += a p ; p = g + (gam'/gam) p
             }
             gam = gam_new;
         }

@@ -81,6 +81,10 @@ int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const Spi
 // fused CG update x += a p ; p = g + b p (x in precision px, p and g in precision pp)
 int mdwf_launch_xpupdate(Prec px, const SpinorBuf &x, double a, Prec pp, const SpinorBuf &p, double b, const SpinorBuf &g,
                          int L5, int Vh, cudaStream_t st);
+// 16-bit Krylov vectors: x += a p ; pnew = g + b p ; bp = (b5 + c5 Lambda) pnew   (p is not overwritten)
+int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g,
+                           const SpinorBuf &pnew, const SpinorBuf &bp, double b5, double c5, double mf, int L5, int Vh,
+                           cudaStream_t st);
 int mdwf_reduce_max_blocks();
 // fixed-order sum of n partials into *result_dev (second pass of every reduction)
 int mdwf_launch_final_sum(const double *partial, int n, double *result_dev, cudaStream_t st);
