@@ -76,6 +76,8 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *   "kernels"         "v3" (default) | "v4" | "v2": kernel family for fp32 arithmetic. v3: hop3_kernels.cuh; v4: the same
  *                     arithmetic with the neighbour groups staged in shared memory by bulk-asynchronous copies
  *                     (Lx = 32, L5 in {8,12} only, else v3); v2: hop_kernels.cuh (always used for fp64 and other L5).
+ *   "bp_stream"       "1" (default) | "0": 16-bit Krylov vectors only -- the fused CG update also writes B p, which K1 of
+ *                     the next Mpc reads instead of applying B on load.
  *   "sweep_mb"        L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
  *   "matpc"           "asym" only (the operator Chroma uses).
  */
@@ -113,7 +115,9 @@ int mdwf_get_stat(const mdwf_ctx *ctx, const char *key, double *value);
 /* Measurement: run op (MDWF_OP_MPC or MDWF_OP_MPCDAG) `reps` times after `warmup`
  * untimed runs, in precision "fp64" | "fp32" | "half", on library-owned hash-filled vectors, timed with
  * CUDA events on the context's stream.  out4[0] = ms per application (both kernels), out4[1] / out4[2] =
- * ms per launch of its first / second kernel timed alone, out4[3] = kernels launched by this call. */
+ * ms per launch of its first / second kernel timed alone, out4[3] = kernels launched by this call.  For the 16-bit
+ * Mpc the first kernel is the one mdwf_solve launches (K1 reading the B p stream of the fused CG update), unless the
+ * option "bp_stream" is "0". */
 int mdwf_time_op(mdwf_ctx *ctx, int op, const char *precision, int reps, int warmup, double *out4);
 
 /* Measurement of the ALU roofline denominators: the device's fp32 fused-multiply-add

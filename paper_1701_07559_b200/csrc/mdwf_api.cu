@@ -801,7 +801,9 @@ int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmu
     for (int phase = 0; phase < 3; phase++) {     // 0: K1 + K2 back to back, 1: K1 alone, 2: K2 alone
         for (int it = -warmup; it < reps; it++) {
             if (it == 0) CUDA_OK(c, cudaEventRecord(e0, c->st));
-            if (phase != 2) TRY(op == MDWF_OP_MPC ? op_Mpc_k1(c, p, a, t) : op_Mpcdag_k1(c, p, a, t));
+            // 16-bit Mpc: time the K1 the CG really launches (it reads the B p stream of the fused update)
+            const bool k1b = (op == MDWF_OP_MPC) && p == PREC_H && c->use_bp && fused_norm_available(c, p);
+            if (phase != 2) TRY(op == MDWF_OP_MPC ? (k1b ? op_Mpc_k1_from_B(c, p, a, t) : op_Mpc_k1(c, p, a, t)) : op_Mpcdag_k1(c, p, a, t));
             if (phase != 1) TRY(op == MDWF_OP_MPC ? op_Mpc_k2(c, p, a, t, b) : op_Mpcdag_k2(c, p, a, t, b));
         }
         CUDA_OK(c, cudaEventRecord(e1, c->st));
