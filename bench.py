@@ -294,9 +294,10 @@ def main():
     alu = {"achieved": k_flops_site * h / (k_ms * 1e-3) / 1e12, "peak": 2 * ffma2, "unit": "TFLOP/s",
            "peak_source": "measured live: packed FFMA2 stream on all SMs (mdwf_fma_rates); scalar FFMA gives %.1f" % (2 * ffma)}
     alu["frac"] = alu["achieved"] / alu["peak"]
-    if sloppy == "half":
-        # 16-bit storage: ncu shows this kernel instruction/ALU-bound: 11.8 counted flop per
-        # algorithmic byte against a machine balance of 10.  The ALU view is the primary one; the HBM view stays beside it.
+    # which ceiling binds this kernel: the larger of its two ideal times
+    t_hbm = k_bytes / (hbm_peak * 1e9)
+    t_alu = k_flops_site * h / (alu["peak"] * 1e12)
+    if t_alu > t_hbm:
         hbm_view = {k: roofline[k] for k in ("achieved", "peak", "unit", "frac", "peak_source")}
         roofline.update({"bound": "alu", "achieved": alu["achieved"], "peak": alu["peak"], "unit": alu["unit"],
                          "frac": alu["frac"], "peak_source": alu["peak_source"], "hbm": hbm_view})
