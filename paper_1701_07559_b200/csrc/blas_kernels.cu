@@ -255,46 +255,64 @@ xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, cons
 // conversion of its halo slices cost more than this extra 16-bit stream).  p_new of the slices s-1 (upper spins)
 // and s+1 (lower spins) is recomputed from p_old and g; p_old is never overwritten, so there is no race.
 template <class PX, class PP>
-__global__ void __launch_bounds__(RED_THREADS)
+__global__ void __launch_bounds__(128)
 xpupdate_b_kernel(void *x, float *xn, double a, const void *p, const float *pn, double b, const void *g, const float *gn,
                   void *pnew, float *pnewn, void *bp, float *bpn, float b5, float c5, float mf, int L5, long Vh)
 {
-    const int s = blockIdx.y;
-    const int sm = (s == 0) ? L5 - 1 : s - 1, sp = (s == L5 - 1) ? 0 : s + 1;
-    const float cu = (s == 0) ? -mf * c5 : c5, cl = (s == L5 - 1) ? -mf * c5 : c5;
-    for (long cb = (long)blockIdx.x * RED_THREADS + threadIdx.x; cb < Vh; cb += (long)gridDim.x * RED_THREADS) {
-        typename PP::R vp[24], vg[24], hp[12], hg[12];
-        typename PX::R vx[24];
+    // one thread walks the L5 slices of one 4D site, so every slice of p and g is loaded once: the new p of slice
+    // s+1 is formed one step ahead, its lower spins feed B at s and its upper spins feed B at s+2
+    using T = typename CompT<PX, PP, PP>::T;
+    using RP = typename PP::R;
+    const long cb = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= Vh) return;
+    const T ta = (T)a, tb = (T)b;
+    RP cur[24], nxt[24], prev_up[12], first_low[12], vp[24], vg[24];
+    auto new_p = [&](int s, RP *out, bool update_x) {
         load_spinor<PP>(p, pn, L5, s, cb, vp);
         load_spinor<PP>(g, gn, L5, s, cb, vg);
-        load_spinor<PX>(x, xn, L5, s, cb, vx);
-        using T = typename CompT<PX, PP, PP>::T;
-        const T ta = (T)a, tb = (T)b;
-        typename PP::R vb[24];
+        if (update_x) {
+            typename PX::R vx[24];
+            load_spinor<PX>(x, xn, L5, s, cb, vx);
 #pragma unroll
-        for (int k = 0; k < 24; k++) {
-            vx[k] = (typename PX::R)((T)vx[k] + ta * (T)vp[k]);
-            vp[k] = (typename PP::R)((T)vg[k] + tb * (T)vp[k]);
+            for (int k = 0; k < 24; k++) vx[k] = (typename PX::R)((T)vx[k] + ta * (T)vp[k]);
+            store_spinor<PX>(x, xn, L5, s, cb, vx);
         }
-        load_half<PP>(p, pn, L5, sm, cb, 0, hp);
-        load_half<PP>(g, gn, L5, sm, cb, 0, hg);
 #pragma unroll
-        for (int k = 0; k < 12; k++) vb[k] = (typename PP::R)(b5 * (float)vp[k] + cu * (float)((T)hg[k] + tb * (T)hp[k]));
-        load_half<PP>(p, pn, L5, sp, cb, 1, hp);
-        load_half<PP>(g, gn, L5, sp, cb, 1, hg);
+        for (int k = 0; k < 24; k++) out[k] = (RP)((T)vg[k] + tb * (T)vp[k]);
+    };
+    {   // upper spins of the new p at slice L5-1 (wall neighbour of slice 0)
+        RP hp[12], hg[12];
+        load_half<PP>(p, pn, L5, L5 - 1, cb, 0, hp);
+        load_half<PP>(g, gn, L5, L5 - 1, cb, 0, hg);
 #pragma unroll
-        for (int k = 0; k < 12; k++) vb[12 + k] = (typename PP::R)(b5 * (float)vp[12 + k] + cl * (float)((T)hg[k] + tb * (T)hp[k]));
-        store_spinor<PX>(x, xn, L5, s, cb, vx);
-        store_spinor<PP>(pnew, pnewn, L5, s, cb, vp);
+        for (int k = 0; k < 12; k++) prev_up[k] = (RP)((T)hg[k] + tb * (T)hp[k]);
+    }
+    new_p(0, cur, true);
+#pragma unroll
+    for (int k = 0; k < 12; k++) first_low[k] = cur[12 + k];
+    for (int s = 0; s < L5; s++) {
+        if (s + 1 < L5) new_p(s + 1, nxt, true);
+        const float cu = (s == 0) ? -mf * c5 : c5, cl = (s == L5 - 1) ? -mf * c5 : c5;
+        RP vb[24];
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            vb[k] = (RP)(b5 * (float)cur[k] + cu * (float)prev_up[k]);
+            vb[12 + k] = (RP)(b5 * (float)cur[12 + k] + cl * (float)((s + 1 < L5) ? nxt[12 + k] : first_low[k]));
+        }
+        store_spinor<PP>(pnew, pnewn, L5, s, cb, cur);
         store_spinor<PP>(bp, bpn, L5, s, cb, vb);
+#pragma unroll
+        for (int k = 0; k < 12; k++) prev_up[k] = cur[k];
+#pragma unroll
+        for (int k = 0; k < 24; k++) cur[k] = nxt[k];
     }
 }
 int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g,
                            const SpinorBuf &pnew, const SpinorBuf &bp, double b5, double c5, double mf, int L5, int Vh,
                            cudaStream_t st)
 {
-    const dim3 nb = site_grid(L5, Vh);
-#define XB(PX) xpupdate_b_kernel<PX, PH><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, pnew.v, \
+    const int nb = (Vh + 127) / 128;
+#define XB(PX) xpupdate_b_kernel<PX, PH><<<nb, 128, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, pnew.v, \
                                                                      pnew.norm, bp.v, bp.norm, (float)b5, (float)c5, (float)mf, L5, Vh)
     if (px == PREC_S) XB(PS);
     else if (px == PREC_H) XB(PH);
