@@ -20,6 +20,7 @@ int mdwf_launch_hop4_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop4_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_sdense_mma(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_S(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
@@ -46,7 +47,10 @@ int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const Spinor
                        cudaStream_t st)
 {
     switch (p) {
-    case PREC_D: return mdwf_launch_sdense_D(L5, Vh, in, out, dense, st);
+    case PREC_D: {   // fp64: tensor-core (DMMA) contraction for L5 <= 16, FMA kernel beyond
+        const int rc = mdwf_launch_sdense_mma(L5, Vh, in, out, dense, st);
+        return rc != -1 ? rc : mdwf_launch_sdense_D(L5, Vh, in, out, dense, st);
+    }
     case PREC_S: return mdwf_launch_sdense_S(L5, Vh, in, out, dense, st);
     default: return mdwf_launch_sdense_H(L5, Vh, in, out, dense, st);
     }

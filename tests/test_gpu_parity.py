@@ -114,6 +114,17 @@ def test_solve_true_residual_by_oracle(name, ladder):
     m.close()
 
 
+@pytest.mark.parametrize("name", ["l5_16", "l5_24", "lx32"])
+def test_solve_other_L5(name):
+    """L5 = 16 (four k-blocks of the tensor-core A^-1), L5 = 24 (FMA fall-back), Lx = 32 with L5 = 12"""
+    orc, m, b = setup(name)
+    m.set_option("ladder", "dsh")
+    sol, iters, tr, rc = m.solve(torch.from_numpy(b).cuda(), tol=1e-10, maxiter=5000)
+    assert rc == 0
+    assert orc.true_residual(b, sol.cpu().numpy()) <= 1e-10
+    m.close()
+
+
 def test_solve_host_buffers_and_point_source():
     from paper_1701_07559_b200 import inputs
     orc, m, _ = setup("cfg1")
