@@ -19,6 +19,10 @@ CASES = {
     "l5_16": ((2, 2, 4, 4), 16, 1.3, 1.75, 0.75, 0.00712, 0.2, 5),     # a15m220 row of Table II
     "l5_24": ((2, 2, 2, 4), 24, 1.3, 2.25, 1.25, 0.00216, 0.2, 6),     # a15m130 row of Table II (generic path)
     "lx32": ((32, 4, 2, 4), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 7),         # Lx = 32: the geometry the v4 (staged) kernels cover
+    "l5_2": ((2, 2, 2, 2), 2, 1.3, 1.5, 0.5, 0.05, 0.3, 12),           # smallest lattice and smallest L5 the ABI accepts
+    "l5_32": ((2, 2, 2, 2), 32, 1.3, 1.5, 0.5, 0.05, 0.3, 13),         # largest L5 the ABI accepts
+    "shamir": ((4, 4, 2, 2), 8, 1.8, 1.0, 0.0, 0.0, 0.3, 14),          # c5 = 0 (B = 1, kappa = -1/alpha), m_f = 0
+    "kappa1": ((4, 4, 2, 2), 8, 1.3, 0.001, 0.0, 0.05, 0.3, 15),       # |kappa| = 0.997: recurrence refused, dense table used
 }
 TOL = {"fp64": 1e-12, "fp32": 1e-5, "half": 2e-3}
 
