@@ -129,6 +129,19 @@ def test_solve_other_L5(name):
     m.close()
 
 
+@pytest.mark.parametrize("name,ladder", [("cfg1", "dsh"), ("lx32", "dsh"), ("ragged", "ds")])
+def test_solve_is_bit_reproducible(name, ladder):
+    """fixed-order reductions everywhere (BLAS-1, fused norms of the hop epilogues): two solves agree bit for bit"""
+    orc, m, b = setup(name)
+    m.set_option("ladder", ladder)
+    src = torch.from_numpy(b).cuda()
+    sol1, it1, tr1, rc1 = m.solve(src, tol=1e-10, maxiter=5000)
+    sol2, it2, tr2, rc2 = m.solve(src, tol=1e-10, maxiter=5000)
+    assert rc1 == 0 and rc2 == 0 and it1 == it2 and tr1 == tr2
+    assert torch.equal(sol1, sol2)
+    m.close()
+
+
 def test_solve_host_buffers_and_point_source():
     from paper_1701_07559_b200 import inputs
     orc, m, _ = setup("cfg1")
