@@ -6,9 +6,9 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdwf_b200.so")
-SOURCES = ["mdwf_api.cu", "hop_d.cu", "hop_s.cu", "hop_h.cu", "hop3_s.cu", "hop3_h.cu", "hop4_s.cu", "hop4_h.cu", "blas_kernels.cu", "layout_kernels.cu", "peak_kernels.cu", "sdense_mma.cu"]
+SOURCES = ["mdwf_api.cu", "hop_d.cu", "hop_s.cu", "hop_h.cu", "hop3_s.cu", "hop3_h.cu", "blas_kernels.cu", "layout_kernels.cu", "peak_kernels.cu", "sdense_mma.cu"]
 FLAGS = os.environ.get("MDWF_NVCC_EXTRA", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+         "-Xcompiler", "-fPIC"]
 
 
 def _deps_mtime():
@@ -21,7 +21,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
-    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")]
+    flags = FLAGS
 
     def compile_one(src):
         obj = os.path.join(objdir, src.replace(".cu", ".o"))

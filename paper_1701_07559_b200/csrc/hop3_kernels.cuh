@@ -36,14 +36,16 @@ MDWF_DEV c2 mk(float a, float b) { return make_float2(a, b); }
 
 // ---- spinor chunk loads into complex pairs ------------------------------------------------------
 // PS: chunk j = float4 = complexes 2j, 2j+1.  PH: chunk j = short4, value = scale * int16.
+// G = true: global memory (read-only path); G = false: a neighbour group staged in shared memory by the copy engine
+template <bool G, class T> MDWF_DEV T ldx(const T *p) { if (G) return __ldg(p); else return *p; }
 template <class P> struct Ld;
 template <> struct Ld<PS> {
     // NC complexes (NC even) from chunk pointer p (stride 32 chunks)
-    template <int NC> static MDWF_DEV void chunks(const float4 *p, float, c2 *v)
+    template <int NC, bool G = true> static MDWF_DEV void chunks(const float4 *p, float, c2 *v)
     {
 #pragma unroll
         for (int j = 0; j < NC / 2; j++) {
-            const float4 q = __ldg(p + 32 * j);
+            const float4 q = ldx<G>(p + 32 * j);
             v[2 * j] = mk(q.x, q.y);
             v[2 * j + 1] = mk(q.z, q.w);
         }
@@ -59,23 +61,23 @@ MDWF_DEV c2 cvt_raw(unsigned w)                // w = two 16-bit values (low hal
 }
 MDWF_DEV c2 cvt_pair(unsigned w, c2 sc) { return mul2(cvt_raw(w), sc); }
 template <> struct Ld<PH> {
-    template <int NC> static MDWF_DEV void chunks(const short4 *p, float sc, c2 *v)
+    template <int NC, bool G = true> static MDWF_DEV void chunks(const short4 *p, float sc, c2 *v)
     {
         const c2 s2 = dup(sc);
 #pragma unroll
         for (int j = 0; j < NC / 2; j++) {
-            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p + 32 * j));
+            const uint2 q = ldx<G>(reinterpret_cast<const uint2 *>(p + 32 * j));
             v[2 * j] = cvt_pair(q.x, s2);
             v[2 * j + 1] = cvt_pair(q.y, s2);
         }
     }
     // the stored integers as floats, unscaled: the hop is linear, so the scale of the slice is applied once, in the
     // reconstruction FMAs (saves one FMUL2 per complex on every neighbour load without B-on-load)
-    template <int NC> static MDWF_DEV void raw(const short4 *p, c2 *v)
+    template <int NC, bool G = true> static MDWF_DEV void raw(const short4 *p, c2 *v)
     {
 #pragma unroll
         for (int j = 0; j < NC / 2; j++) {
-            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p + 32 * j));
+            const uint2 q = ldx<G>(reinterpret_cast<const uint2 *>(p + 32 * j));
             v[2 * j] = cvt_raw(q.x);
             v[2 * j + 1] = cvt_raw(q.y);
         }
@@ -98,48 +100,51 @@ MDWF_DEV void gget(const short2 q, float &re, float &im)
     re = v.x;
     im = v.y;
 }
-// Build one link ONCE per block: load it as stored (6 or 9 complex chunks), rebuild row 2 for 12-real storage,
-// take the dagger for a backward hop, and write the 9 complex entries of this lane to the block's shared-memory
-// link table (element k at dst[32 k]).
-template <class P, bool DAGGER>
-MDWF_DEV void stage_link(const void *gbase, int mu, long cb, int recon, float2 *dst)
+// The link tile of the block's 32 sites ([8 directions][NK][32] in the gauge layout, backward links already pulled back
+// and daggered) is brought into shared memory by ONE bulk copy of the TMA engine (hop3_kernel).  expand_link finishes
+// direction d of this lane in the link table sL (element k at sL[(d*9 + k)*32 + lane]):
+//   fp32 storage : the copy lands in the table itself; with 12-real storage row 2 = conj(row0 x row1) is added in place;
+//   16-bit       : the raw tile lands in sR, is converted (and completed) here.
+MDWF_DEV void row2_from_rows01(float *ur, float *ui)
 {
-    using G = typename P::G;
-    const int NK = recon >> 1;
-    const G *p = reinterpret_cast<const G *>(gbase) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
-    G raw[9];
+    // row2[c] = conj(row0[a] row1[b] - row0[b] row1[a]),  (a,b) = (c+1, c+2) mod 3
 #pragma unroll
-    for (int k = 0; k < 6; k++) raw[k] = __ldg(p + 32 * k);
-    if (recon == 18) {
-#pragma unroll
-        for (int k = 6; k < 9; k++) raw[k] = __ldg(p + 32 * k);
+    for (int c = 0; c < 3; c++) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        float re = ur[a] * ur[3 + b];
+        re = fmaf(-ui[a], ui[3 + b], re); re = fmaf(-ur[b], ur[3 + a], re); re = fmaf(ui[b], ui[3 + a], re);
+        float im = ur[a] * ui[3 + b];
+        im = fmaf(ui[a], ur[3 + b], im); im = fmaf(-ur[b], ui[3 + a], im); im = fmaf(-ui[b], ur[3 + a], im);
+        ur[6 + c] = re;
+        ui[6 + c] = -im;
     }
+}
+template <class P>
+MDWF_DEV void expand_link(const void *sR, float2 *sL, int d, int lane, int recon)
+{
     float ur[9], ui[9];
+    float2 *row = sL + d * 288 + lane;
+    if (!P::HALF) {
+        if (recon == 18) return;
 #pragma unroll
-    for (int k = 0; k < 6; k++) gget(raw[k], ur[k], ui[k]);
-    if (recon == 18) {
+        for (int k = 0; k < 6; k++) gget(row[32 * k], ur[k], ui[k]);
+        row2_from_rows01(ur, ui);
 #pragma unroll
-        for (int k = 6; k < 9; k++) gget(raw[k], ur[k], ui[k]);
+        for (int k = 6; k < 9; k++) row[32 * k] = make_float2(ur[k], ui[k]);
     } else {
-        // row2[c] = conj(row0[a] row1[b] - row0[b] row1[a]),  (a,b) = (c+1, c+2) mod 3
+        const int NK = recon >> 1;
+        const short2 *raw = reinterpret_cast<const short2 *>(sR) + d * NK * 32 + lane;
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
-            const int a = (c + 1) % 3, b = (c + 2) % 3;
-            float re = ur[a] * ur[3 + b];
-            re = fmaf(-ui[a], ui[3 + b], re); re = fmaf(-ur[b], ur[3 + a], re); re = fmaf(ui[b], ui[3 + a], re);
-            float im = ur[a] * ui[3 + b];
-            im = fmaf(ui[a], ur[3 + b], im); im = fmaf(-ur[b], ui[3 + a], im); im = fmaf(-ui[b], ur[3 + a], im);
-            ur[6 + c] = re;
-            ui[6 + c] = -im;
+        for (int k = 0; k < 6; k++) gget(raw[32 * k], ur[k], ui[k]);
+        if (recon == 18) {
+#pragma unroll
+            for (int k = 6; k < 9; k++) gget(raw[32 * k], ur[k], ui[k]);
+        } else {
+            row2_from_rows01(ur, ui);
         }
+#pragma unroll
+        for (int k = 0; k < 9; k++) row[32 * k] = make_float2(ur[k], ui[k]);
     }
-#pragma unroll
-    for (int a = 0; a < 3; a++)
-#pragma unroll
-        for (int c = 0; c < 3; c++) {
-            if (!DAGGER) dst[32 * (a * 3 + c)] = make_float2(ur[a * 3 + c], ui[a * 3 + c]);
-            else dst[32 * (a * 3 + c)] = make_float2(ur[c * 3 + a], -ui[c * 3 + a]);   // conj(U_ca)
-        }
 }
 // p = this lane's column of the shared-memory link table of one direction
 MDWF_DEV void load_link3(const float2 *p, Link &L)
@@ -236,31 +241,38 @@ MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
 // PRE = 1 applies (1 + f Lambda) to the neighbour on load: upper spins add f * (slice s-1), lower spins
 // f * (slice s+1), wall factor -m_f at the wrap.  The window slides over the S slices (one half-spinor of
 // halo on each side), so only one full slice and two half slices are live at a time.
-template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR>
-MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, long cb_nb, float bsign,
-                        c2 (*acc)[12], long cb_pf = -1)
+// gb / nb: chunk 0 of slice 0 and scale of slice 0 of this thread's neighbour site; slice s is at gb + s*32*NV, nb + 32 s,
+// in global memory (G = true) as well as in a staged group (G = false), which keeps the [s][chunk][lane] layout.
+template <class P, bool G> MDWF_DEV float ld_scale(const float *np)
+{
+    if (!P::HALF) return 1.0f;
+    return ldx<G>(np) * (1.0f / MDWF_FIXED_MAX);
+}
+template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR, bool G>
+MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const typename P::V *gb, const float *nb, float bsign,
+                        c2 (*acc)[12])
 {
     using V = typename P::V;
     constexpr int SGN = (FWD ? 1 : -1) * (DAG ? -1 : 1);
     Link U;
     load_link3(sl, U);
 
-    const V *p0 = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, s0);
-    const long n0 = sp_noff(L5, cb_nb, s0);
     constexpr long SL = 32 * P::NV;
+    const V *p0 = gb + s0 * SL;
+    const float *n0 = nb + 32 * s0;
 
     if (PRE == 0) {
 #pragma unroll
         for (int k = 0; k < S; k++) {
             c2 v[12], h[6], chi[6];
             if constexpr (P::HALF) {
-                const float sck = load_scale<P>(a.in_norm, n0 + 32 * k);
-                Ld<P>::template raw<12>(p0 + k * SL, v);
+                const float sck = ld_scale<P, G>(n0 + 32 * k);
+                Ld<P>::template raw<12, G>(p0 + k * SL, v);
                 project3<MU, SGN>(v, h);
                 su3_mul3(U, h, chi);
                 recon3<MU, SGN, true>(chi, TDIR ? bsign * sck : sck, acc[k]);
             } else {
-                Ld<P>::template chunks<12>(p0 + k * SL, load_scale<P>(a.in_norm, n0 + 32 * k), v);
+                Ld<P>::template chunks<12, G>(p0 + k * SL, 1.0f, v);
                 project3<MU, SGN>(v, h);
                 su3_mul3(U, h, chi);
                 recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
@@ -271,18 +283,14 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, long 
         const int sm = (s0 == 0) ? L5 - 1 : s0 - 1;
         const int sp = (s0 + S >= L5) ? 0 : s0 + S;
         c2 prev_up[6], cur[12], nxt[12];
-        {
-            const V *pm = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, sm);
-            Ld<P>::template chunks<6>(pm, load_scale<P>(a.in_norm, sp_noff(L5, cb_nb, sm)), prev_up);
-        }
-        Ld<P>::template chunks<12>(p0, load_scale<P>(a.in_norm, n0), cur);
+        Ld<P>::template chunks<6, G>(gb + sm * SL, ld_scale<P, G>(nb + 32 * sm), prev_up);
+        Ld<P>::template chunks<12, G>(p0, ld_scale<P, G>(n0), cur);
 #pragma unroll
         for (int k = 0; k < S; k++) {
             if (k < S - 1) {
-                Ld<P>::template chunks<12>(p0 + (k + 1) * SL, load_scale<P>(a.in_norm, n0 + 32 * (k + 1)), nxt);
+                Ld<P>::template chunks<12, G>(p0 + (k + 1) * SL, ld_scale<P, G>(n0 + 32 * (k + 1)), nxt);
             } else {
-                const V *pp = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, sp) + 32 * (P::NV / 2);
-                Ld<P>::template chunks<6>(pp, load_scale<P>(a.in_norm, sp_noff(L5, cb_nb, sp)), nxt + 6);
+                Ld<P>::template chunks<6, G>(gb + sp * SL + 32 * (P::NV / 2), ld_scale<P, G>(nb + 32 * sp), nxt + 6);
             }
             const c2 fu = dup((s0 + k == 0) ? fw : f);
             const c2 fl = dup((s0 + k == L5 - 1) ? fw : f);
@@ -400,9 +408,9 @@ template <class P, int S> struct Hop3Cfg {
     static constexpr int WARPS = P::HALF ? MDWF_H3_WARPS_H : MDWF_H3_WARPS;
 };
 
-// ---- epilogue shared by the v3 and v4 kernels: fifth-dimension POST step, own-site term, store, fused norm ----
+// ---- epilogue shared by the v3 and v5 kernels: fifth-dimension POST step, own-site term, store, fused norm ----
 template <class P, int DAG, int POST, int OWN, int L5, int S>
-MDWF_DEV void epilogue3(const HopArgs &a, c2 (*acc)[12], c2 *sE, int lane, int sg, int s0, long cb, bool active)
+MDWF_DEV void epilogue3(const HopArgs &a, c2 (*acc)[12], c2 *sE, int lane, int sg, int s0, long cb, bool active, int pidx)
 {
     constexpr int NSG = L5 / S;
     using V = typename P::V;
@@ -502,30 +510,122 @@ MDWF_DEV void epilogue3(const HopArgs &a, c2 (*acc)[12], c2 *sE, int lane, int s
             double t = 0.0;
 #pragma unroll
             for (int j = 0; j < NSG; j++) t += wsum[j];
-            a.partial[blockIdx.x] = t;
+            a.partial[pidx] = t;                     // pidx = index of the 32-site group in the sweep order
         }
     }
 }
 
-template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+// ---- bulk-asynchronous copies (TMA engine) and their barriers ------------------------------------------------
+MDWF_DEV unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+MDWF_DEV void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%1], %0;" ::"r"(count), "r"(smem_u32(bar)) : "memory");
+}
+MDWF_DEV void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%1], %0;" ::"r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+MDWF_DEV void mbar_wait(unsigned long long *bar, unsigned phase)
+{
+    unsigned ok = 0;
+    const unsigned addr = smem_u32(bar);
+    while (!ok) {
+        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.u32 %0, 1, 0, P1;\n\t}"
+                     : "=r"(ok)
+                     : "r"(addr), "r"(phase)
+                     : "memory");
+    }
+}
+MDWF_DEV void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+MDWF_DEV void bulk_prefetch_l2(const void *src_gmem, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+MDWF_DEV unsigned fdiv(unsigned n, const FastDiv &f) { return f.m ? (__umulhi(n, f.m) >> f.s) : n; }
+
+// NST = number of neighbour groups STAGED IN SHARED MEMORY BY THE TMA ENGINE (0, 2: t+-, 4: z+- and t+-).
+// Why (profiles/r02_l2_sm_ceiling.md): L2 delivers 34 TB/s to LDG and >= 22 TB/s to bulk copies on this B200, so the
+// ~10 TB/s the all-LDG kernel pulls is not a delivery cap -- 8 warps of ~250 registers cannot keep more than ~70 KB of
+// loads in flight per SM.  The z+- / t+- neighbours of a 32-site group are whole groups (one contiguous
+// L5*NV*512 B slab each, same lane), nothing else on the SM reuses them, and the block's shared memory is otherwise
+// idle: one elected thread starts their bulk copies (cp.async.bulk, completion on an mbarrier) before the links are
+// staged, the x / y directions stream through registers and L1 as before, and by the time the block reaches the
+// staged directions their data is in shared memory.  Bytes in flight per SM: registers + NST * 37 KB per block.
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S, int NST>
 __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S) > 0 ? Hop3Cfg<P, S>::WARPS / (L5 / S) : 1) hop3_kernel(const HopArgs a)
 {
-    constexpr int NSG = L5 / S;
+    constexpr int NSG = L5 / S, NV = P::NV;
     using V = typename P::V;
-    extern __shared__ __align__(16) unsigned char smem_raw3[];
-    c2 *sE = reinterpret_cast<c2 *>(smem_raw3);          // [NSG][12][32] carries / halo slices (POST != 0)
-    float2 *sL = reinterpret_cast<float2 *>(smem_raw3 + (POST != 0 ? NSG * 12 * 32 * sizeof(c2) : 0));   // [8][9][32] links
+    constexpr unsigned BUF_BYTES = L5 * NV * 32 * sizeof(V);          // one staged group
+    constexpr unsigned NRM_BYTES = P::HALF ? L5 * 32 * sizeof(float) : 0;
+    constexpr unsigned SLOT_BYTES = BUF_BYTES + NRM_BYTES;
+    constexpr unsigned SE_BYTES = (POST != 0) ? NSG * 12 * 32 * sizeof(c2) : 0;
+    using G = typename P::G;
+    constexpr unsigned SL_BYTES = 8 * 9 * 32 * sizeof(float2);
+    constexpr unsigned SR_BYTES = P::HALF ? 8 * 9 * 32 * sizeof(short2) : 0;
+    extern __shared__ __align__(128) unsigned char smem_raw3[];
+    unsigned char *rest = smem_raw3 + NST * SLOT_BYTES;                // staged groups first (128-byte aligned slabs)
+    c2 *sE = reinterpret_cast<c2 *>(rest);                             // [NSG][12][32] carries / halo slices (POST != 0)
+    float2 *sL = reinterpret_cast<float2 *>(rest + SE_BYTES);          // [8][9][32] link table
+    unsigned char *sR = rest + SE_BYTES + SL_BYTES;                    // 16-bit storage: the raw link tile
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(sR + SR_BYTES);   // [1 + NST]: link tile, staged groups
     const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
+    const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
+    const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
     long cb0 = (long)blockIdx.x * 32;
     if (a.sweep_nb) {                                    // z-chunked t sweep, see hop_kernels.cuh
-        const int Lt = a.L[3];
-        const int per_chunk = a.sweep_nb * Lt;
-        const int c = blockIdx.x / per_chunk, r = blockIdx.x - c * per_chunk;
-        const int t = r / a.sweep_nb, q = r - t * a.sweep_nb;
-        cb0 = (long)t * ((long)a.Vh / Lt) + (long)c * a.sweep_chunk + (long)q * 32;
+        const unsigned c = fdiv(blockIdx.x, a.dchunk), r = blockIdx.x - c * (unsigned)(a.sweep_nb * Lt);
+        const unsigned t = fdiv(r, a.dnb), q = r - t * (unsigned)a.sweep_nb;
+        cb0 = (long)t * st + (long)c * a.sweep_chunk + (long)q * 32;
     }
     const long cb = cb0 + lane;
     const bool active = cb < a.Vh;
+
+    // ---- one elected thread starts the bulk copies: the link tile of the 32 sites, then the staged neighbour groups ----
+    if (lane == 0 && sg == 0) {
+#pragma unroll
+        for (int k = 0; k < 1 + NST; k++) mbar_init(&bar[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const int NK = a.recon >> 1;
+        const G *tile = reinterpret_cast<const G *>(a.gauge) + (cb0 >> 5) * (long)(8 * NK * 32);
+        mbar_expect_tx(&bar[0], 8 * NK * 32 * sizeof(G));
+        if (P::HALF || NK == 9) {
+            bulk_g2s(P::HALF ? (void *)sR : (void *)sL, tile, 8 * NK * 32 * sizeof(G), &bar[0]);
+        } else {
+#pragma unroll
+            for (int d = 0; d < 8; d++) bulk_g2s(sL + d * 288, tile + d * 6 * 32, 6 * 32 * sizeof(G), &bar[0]);   // rows 0,1 of each direction
+        }
+        if (OWN != 0) {     // the own-site slab the epilogue reads: pull it into L2 now
+            bulk_prefetch_l2(reinterpret_cast<const V *>(a.own) + (cb0 >> 5) * (long)(L5 * NV * 32), BUF_BYTES);
+            if (P::HALF) bulk_prefetch_l2(a.own_norm + (cb0 >> 5) * (long)(L5 * 32), NRM_BYTES);
+        }
+        if (NST > 0) {
+            // the launcher guarantees Lxh*Ly % 32 == 0: all 32 sites of the block share (z,t) and their z / t neighbours
+            // are the whole groups at cb0 -+ sz, cb0 -+ st (periodic wrap), lane for lane
+            const unsigned zt = fdiv(fdiv((unsigned)cb0, a.dLxh), a.dLy), t0 = fdiv(zt, a.dLz), z0 = zt - t0 * Lz;
+            long src[4];
+            src[NST - 2] = (t0 == Lt - 1) ? cb0 - (Lt - 1) * st : cb0 + st;
+            src[NST - 1] = (t0 == 0) ? cb0 + (Lt - 1) * st : cb0 - st;
+            if (NST == 4) {
+                src[0] = (z0 == Lz - 1) ? cb0 - (Lz - 1) * sz : cb0 + sz;
+                src[1] = (z0 == 0) ? cb0 + (Lz - 1) * sz : cb0 - sz;
+            }
+#pragma unroll
+            for (int k = 0; k < NST; k++) {
+                unsigned char *dst = smem_raw3 + k * SLOT_BYTES;
+                mbar_expect_tx(&bar[1 + k], SLOT_BYTES);
+                bulk_g2s(dst, reinterpret_cast<const V *>(a.in) + (src[k] >> 5) * (long)(L5 * NV * 32), BUF_BYTES, &bar[1 + k]);
+                if (P::HALF) bulk_g2s(dst + BUF_BYTES, a.in_norm + (src[k] >> 5) * (long)(L5 * 32), NRM_BYTES, &bar[1 + k]);
+            }
+        }
+    }
 
     c2 acc[S][12];
 #pragma unroll
@@ -535,76 +635,111 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
 
     // neighbour indices (inactive lanes of a ragged last block keep cb = 0 and load nothing)
     const long cbs = active ? cb : 0;
-    const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
-    int r = (int)cbs;
-    const int xh = r % Lxh; r /= Lxh;
-    const int y = r % Ly;   r /= Ly;
-    const int z = r % Lz;
-    const int t = r / Lz;
+    const unsigned q1 = fdiv((unsigned)cbs, a.dLxh), q2 = fdiv(q1, a.dLy), q3 = fdiv(q2, a.dLz);
+    const int xh = (int)((unsigned)cbs - q1 * Lxh), y = (int)(q1 - q2 * Ly), z = (int)(q2 - q3 * Lz), t = (int)q3;
     const int xodd = (a.parity_out + y + z + t) & 1;
-    const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
-    long nb[8];
+    long nb[8];                                                  // link-tile order: 0-3 forward mu, 4-7 backward mu
     nb[0] = xodd ? (xh == Lxh - 1 ? cbs - (Lxh - 1) : cbs + 1) : cbs;
-    nb[1] = xodd ? cbs : (xh == 0 ? cbs + (Lxh - 1) : cbs - 1);
-    nb[2] = (y == Ly - 1) ? cbs - (Ly - 1) * sy : cbs + sy;
-    nb[3] = (y == 0) ? cbs + (Ly - 1) * sy : cbs - sy;
-    nb[4] = (z == Lz - 1) ? cbs - (Lz - 1) * sz : cbs + sz;
-    nb[5] = (z == 0) ? cbs + (Lz - 1) * sz : cbs - sz;
-    nb[6] = (t == Lt - 1) ? cbs - (Lt - 1) * st : cbs + st;
+    nb[4] = xodd ? cbs : (xh == 0 ? cbs + (Lxh - 1) : cbs - 1);
+    nb[1] = (y == Ly - 1) ? cbs - (Ly - 1) * sy : cbs + sy;
+    nb[5] = (y == 0) ? cbs + (Ly - 1) * sy : cbs - sy;
+    nb[2] = (z == Lz - 1) ? cbs - (Lz - 1) * sz : cbs + sz;
+    nb[6] = (z == 0) ? cbs + (Lz - 1) * sz : cbs - sz;
+    nb[3] = (t == Lt - 1) ? cbs - (Lt - 1) * st : cbs + st;
     nb[7] = (t == 0) ? cbs + (Lt - 1) * st : cbs - st;
     const float btp = (t == Lt - 1) ? -1.f : 1.f;               // antiperiodic in t
     const float btm = (t == 0) ? -1.f : 1.f;
 
-    // stage the 8 links of the block's 32 sites in shared memory once: direction d = 2 mu + (0 fwd, 1 bwd) is
-    // fetched by warp d mod NSG; the NSG warps of a site then read them from there (no per-direction global
-    // latency on the critical path, 1/NSG of the global link loads)
-    if (active) {
+    // the link tile has landed (its latency ran under the index arithmetic above): warp d mod NSG completes direction d
+    __syncthreads();                                             // barrier initialisation visible to every thread
+    mbar_wait(&bar[0], 0);
 #pragma unroll
-        for (int d = 0; d < 8; d++)
-            if ((d % NSG) == sg) {
-                if ((d & 1) == 0) stage_link<P, false>(a.gauge_same, d >> 1, cbs, a.recon, sL + d * 9 * 32 + lane);
-                else stage_link<P, true>(a.gauge_other, d >> 1, nb[d], a.recon, sL + d * 9 * 32 + lane);
-            }
-    }
+    for (int d = 0; d < 8; d++)
+        if ((d % NSG) == sg) expand_link<P>(sR, sL, d, lane, a.recon);
     __syncthreads();
 
     if (active) {
-        hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, nb[0], 1.f, acc);
-        hop_dir3<P, 0, false, DAG, PRE, S, false>(a, L5, s0, sL + 1 * 288 + lane, nb[1], 1.f, acc);
-        hop_dir3<P, 1, true, DAG, PRE, S, false>(a, L5, s0, sL + 2 * 288 + lane, nb[2], 1.f, acc);
-        hop_dir3<P, 1, false, DAG, PRE, S, false>(a, L5, s0, sL + 3 * 288 + lane, nb[3], 1.f, acc);
-        hop_dir3<P, 2, true, DAG, PRE, S, false>(a, L5, s0, sL + 4 * 288 + lane, nb[4], 1.f, acc);
-        hop_dir3<P, 2, false, DAG, PRE, S, false>(a, L5, s0, sL + 5 * 288 + lane, nb[5], 1.f, acc);
-        hop_dir3<P, 3, true, DAG, PRE, S, true>(a, L5, s0, sL + 6 * 288 + lane, nb[6], btp, acc);
-        hop_dir3<P, 3, false, DAG, PRE, S, true>(a, L5, s0, sL + 7 * 288 + lane, nb[7], btm, acc);
+        const V *gin = reinterpret_cast<const V *>(a.in);
+        // neighbour in global memory: chunk 0 of slice 0 / scale of slice 0 of site nb[d]
+#define MDWF_GDIR(MU, FWD, TD, d, bs) \
+        hop_dir3<P, MU, FWD, DAG, PRE, S, TD, true>(a, L5, s0, sL + (d) * 288 + lane, gin + sp_off(L5, NV, nb[d], 0), \
+                                                    a.in_norm + sp_noff(L5, nb[d], 0), bs, acc)   /* d = FWD ? MU : 4 + MU */
+        // neighbour group staged in slot k: same lane
+#define MDWF_SDIR(MU, FWD, TD, d, bs, k) \
+        do { mbar_wait(&bar[1 + (k)], 0); \
+             hop_dir3<P, MU, FWD, DAG, PRE, S, TD, false>(a, L5, s0, sL + (d) * 288 + lane, \
+                 reinterpret_cast<const V *>(smem_raw3 + (k) * SLOT_BYTES) + lane, \
+                 reinterpret_cast<const float *>(smem_raw3 + (k) * SLOT_BYTES + BUF_BYTES) + lane, bs, acc); } while (0)
+        MDWF_GDIR(0, true, false, 0, 1.f);
+        MDWF_GDIR(0, false, false, 4, 1.f);
+        MDWF_GDIR(1, true, false, 1, 1.f);
+        MDWF_GDIR(1, false, false, 5, 1.f);
+        if (NST == 4) {
+            MDWF_SDIR(2, true, false, 2, 1.f, 0);
+            MDWF_SDIR(2, false, false, 6, 1.f, 1);
+        } else {
+            MDWF_GDIR(2, true, false, 2, 1.f);
+            MDWF_GDIR(2, false, false, 6, 1.f);
+        }
+        if (NST >= 2) {
+            MDWF_SDIR(3, true, true, 3, btp, NST - 2);
+            MDWF_SDIR(3, false, true, 7, btm, NST - 1);
+        } else {
+            MDWF_GDIR(3, true, true, 3, btp);
+            MDWF_GDIR(3, false, true, 7, btm);
+        }
+#undef MDWF_GDIR
+#undef MDWF_SDIR
     }
 
-    epilogue3<P, DAG, POST, OWN, L5, S>(a, acc, sE, lane, sg, s0, cb, active);
+    epilogue3<P, DAG, POST, OWN, L5, S>(a, acc, sE, lane, sg, s0, cb, active, (int)blockIdx.x);
 }
 
 // ---- launchers ----------------------------------------------------------------------------------
-template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S, int NST>
 static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
 {
     constexpr int NSG = L5 / S;
+    using V = typename P::V;
     dim3 block(32, NSG);
     dim3 grid((unsigned)((a.Vh + 31) / 32));
-    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float2);
-    if (smem > 32 * 1024) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
-        cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S>,
+    const size_t smem = (size_t)NST * ((size_t)L5 * P::NV * 32 * sizeof(V) + (P::HALF ? (size_t)L5 * 32 * sizeof(float) : 0)) +
+                        ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float2) +
+                        (P::HALF ? (size_t)8 * 9 * 32 * sizeof(short2) : 0) + 8 * (1 + NST);
+    static bool attr_set = false;                                // once per instantiation, not once per launch
+    if (smem > 32 * 1024 && !attr_set) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
+        cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S, NST>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
+        attr_set = true;
     }
-    hop3_kernel<P, DAG, PRE, POST, OWN, L5, S><<<grid, block, smem, st>>>(a);
+    hop3_kernel<P, DAG, PRE, POST, OWN, L5, S, NST><<<grid, block, smem, st>>>(a);
     return (int)cudaGetLastError();
+}
+// number of neighbour groups the copy engine stages for this launch (0 when the geometry does not allow it)
+template <class P> static inline int hop3_staged(const HopArgs &a)
+{
+    if (a.kver < 4) return 0;                                    // option kernels=v3: every direction through registers
+    const long plane = (long)(a.L[0] >> 1) * a.L[1];
+    if (plane % 32 != 0 || a.Vh % 32 != 0) return 0;             // groups must not straddle (z,t) planes
+    if (a.L[2] < 2 || a.L[3] < 2) return 0;
+    return P::HALF ? MDWF_H3_NST_H : MDWF_H3_NST_S;
+}
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
+static int launch_hop3_nst(const HopArgs &a, cudaStream_t st)
+{
+    const int nst = hop3_staged<P>(a);
+    if (nst == 4) return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, (P::HALF ? 4 : 2)>(a, st);   // fp32 slabs: 2 fit beside a second block
+    if (nst == 2) return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, 2>(a, st);
+    return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, 0>(a, st);
 }
 template <class P, int DAG, int PRE, int POST, int OWN>
 static int launch_hop3_l5(const HopArgs &a, cudaStream_t st)
 {
-    if (a.L5 == 12) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 12, MDWF_H3_S12>(a, st);
+    if (a.L5 == 12) return launch_hop3_nst<P, DAG, PRE, POST, OWN, 12, MDWF_H3_S12>(a, st);
 #ifndef MDWF_DEV_FAST
-    if (a.L5 == 8) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 8, 2>(a, st);
-    if (a.L5 == 16) return launch_hop3_inst<P, DAG, PRE, POST, OWN, 16, 2>(a, st);
+    if (a.L5 == 8) return launch_hop3_nst<P, DAG, PRE, POST, OWN, 8, 2>(a, st);
+    if (a.L5 == 16) return launch_hop3_nst<P, DAG, PRE, POST, OWN, 16, 2>(a, st);
 #endif
     return (int)cudaErrorInvalidValue;
 }

@@ -20,7 +20,8 @@
 #include "mdwf_device.cuh"
 #include "mdwf_internal.h"
 
-// One direction of the stencil for S slices.  FWD: neighbour x+mu with U_mu(x); else x-mu with U_mu(x-mu)^+.
+// One direction of the stencil for S slices.  FWD: neighbour x+mu with U_mu(x); else x-mu with U_mu(x-mu)^+ (link
+// direction 4 + mu of the site's own tile).
 template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR>
 MDWF_DEV void hop_dir(const HopArgs &a, int L5, int s0, long cb_own, long cb_nb, typename P::R bsign,
                       typename P::R (*acc)[24])
@@ -29,8 +30,7 @@ MDWF_DEV void hop_dir(const HopArgs &a, int L5, int s0, long cb_own, long cb_nb,
     using V = typename P::V;
     constexpr int SGN = (FWD ? 1 : -1) * (DAG ? -1 : 1);   // H: (1 - gamma) forward, (1 + gamma) backward
     R U[18];
-    if (FWD) load_link<P>(a.gauge_same, MU, cb_own, a.recon, U);
-    else load_link<P>(a.gauge_other, MU, cb_nb, a.recon, U);
+    load_link<P>(a.gauge, FWD ? MU : 4 + MU, cb_own, a.recon, U);   // backward links are stored pulled back and daggered
 
     const V *p0 = reinterpret_cast<const V *>(a.in) + sp_off(L5, P::NV, cb_nb, s0);   // slice s0, chunk 0
     const long n0 = sp_noff(L5, cb_nb, s0);
@@ -42,7 +42,7 @@ MDWF_DEV void hop_dir(const HopArgs &a, int L5, int s0, long cb_own, long cb_nb,
             R v[24], h[12], chi[12];
             load_chunks_at<P, P::NV>(p0 + k * SL, load_scale<P>(a.in_norm, n0 + 32 * k), v);
             project<MU, SGN>(v, h);
-            if (FWD) su3_mul<false>(U, h, chi); else su3_mul<true>(U, h, chi);
+            su3_mul<false>(U, h, chi);
             recon_add<MU, SGN, TDIR>(chi, bsign, acc[k]);
         }
     } else {
@@ -73,7 +73,7 @@ MDWF_DEV void hop_dir(const HopArgs &a, int L5, int s0, long cb_own, long cb_nb,
                 w[12 + q] = fma(fl, nxt[12 + q], cur[12 + q]);
             }
             project<MU, SGN>(w, h);
-            if (FWD) su3_mul<false>(U, h, chi); else su3_mul<true>(U, h, chi);
+            su3_mul<false>(U, h, chi);
             recon_add<MU, SGN, TDIR>(chi, bsign, acc[k]);
 #pragma unroll
             for (int q = 0; q < 12; q++) prev_up[q] = cur[q];

@@ -11,7 +11,7 @@ size_t mdwf_spinor_bytes(Prec p, int L5, int Vh)
 }
 size_t mdwf_gauge_bytes(Prec p, int Vh, int recon)
 {
-    const size_t n = (size_t)4 * padded(Vh) * recon;
+    const size_t n = (size_t)8 * padded(Vh) * recon;         // 4 forward links + 4 pulled-back backward links per site
     return p == PREC_D ? n * 8 : (p == PREC_S ? n * 4 : n * 2);
 }
 
@@ -71,19 +71,38 @@ MDWF_DEV short2 gpack(double re, double im, short2 *)
                        (short)(unsigned short)(__double2int_rn(im * (double)MDWF_FIXED_MAX) + 32768));
 }
 
+// Link tile of a site x of the given parity, 8 directions d:
+//   d = mu     : U_mu(x)                      (forward hop)
+//   d = 4 + mu : U_mu(x - mu)^dagger          (backward hop, pulled back to x and already daggered)
+// so the 8 links of a 32-site group are ONE contiguous slab [8][NK][32] (one bulk copy per block in the hop kernels).
+// With recon = 12 rows 0 and 1 of the stored matrix are kept (row 2 = conj(row0 x row1) holds for U and for U^dagger).
 template <class P, class T>
-__global__ void gauge_in_kernel(const T *canon, void *dst, long Vh, int parity, int recon, int Lx, int Ly, int Lz)
+__global__ void gauge_in_kernel(const T *canon, void *dst, long Vh, int parity, int recon, int Lx, int Ly, int Lz, int Lt)
 {
     using G = typename P::G;
     const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= 4 * Vh) return;
-    const int mu = (int)(idx / Vh);
-    const long cb = idx - (long)mu * Vh;
-    const long lex = cb_to_lex(cb, parity, Lx, Ly, Lz);
+    if (idx >= 8 * Vh) return;
+    const int d = (int)(idx / Vh), mu = d & 3;
+    const long cb = idx - (long)d * Vh;
+    long lex = cb_to_lex(cb, parity, Lx, Ly, Lz);
+    if (d >= 4) {                                   // site x - mu (periodic; the antiperiodic sign lives in the kernels)
+        long r = lex;
+        const int x = (int)(r % Lx); r /= Lx;
+        const int y = (int)(r % Ly); r /= Ly;
+        const int z = (int)(r % Lz);
+        const int t = (int)(r / Lz);
+        const int xm = (mu == 0) ? (x + Lx - 1) % Lx : x, ym = (mu == 1) ? (y + Ly - 1) % Ly : y;
+        const int zm = (mu == 2) ? (z + Lz - 1) % Lz : z, tm = (mu == 3) ? (t + Lt - 1) % Lt : t;
+        lex = xm + (long)Lx * (ym + (long)Ly * (zm + (long)Lz * tm));
+    }
     const T *p = canon + (lex * 4 + mu) * 18;
     const int NK = recon >> 1;
-    G *q = reinterpret_cast<G *>(dst) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
-    for (int k = 0; k < NK; k++) q[32 * k] = gpack((double)p[2 * k], (double)p[2 * k + 1], (G *)nullptr);
+    G *q = reinterpret_cast<G *>(dst) + ((((cb >> 5) * 8 + d) * NK) << 5) + (cb & 31);
+    for (int k = 0; k < NK; k++) {
+        const int a = k / 3, c = k - 3 * a;
+        if (d < 4) q[32 * k] = gpack((double)p[2 * k], (double)p[2 * k + 1], (G *)nullptr);
+        else q[32 * k] = gpack((double)p[2 * (c * 3 + a)], -(double)p[2 * (c * 3 + a) + 1], (G *)nullptr);   // conj(U_ca)
+    }
 }
 
 template <class P>
@@ -160,11 +179,11 @@ static int gauge_in(const void *canon, int real_bytes, void *dst, const int *L, 
 {
     const long Vh = (long)L[0] * L[1] * L[2] * L[3] / 2;
     const int T = 128;
-    const unsigned nb = (unsigned)((4 * Vh + T - 1) / T);
+    const unsigned nb = (unsigned)((8 * Vh + T - 1) / T);
     if (real_bytes == 8)
-        gauge_in_kernel<P, double><<<nb, T, 0, st>>>((const double *)canon, dst, Vh, parity, recon, L[0], L[1], L[2]);
+        gauge_in_kernel<P, double><<<nb, T, 0, st>>>((const double *)canon, dst, Vh, parity, recon, L[0], L[1], L[2], L[3]);
     else
-        gauge_in_kernel<P, float><<<nb, T, 0, st>>>((const float *)canon, dst, Vh, parity, recon, L[0], L[1], L[2]);
+        gauge_in_kernel<P, float><<<nb, T, 0, st>>>((const float *)canon, dst, Vh, parity, recon, L[0], L[1], L[2], L[3]);
     return (int)cudaGetLastError();
 }
 int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, const int *L, int parity, int recon,

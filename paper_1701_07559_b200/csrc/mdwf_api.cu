@@ -16,8 +16,6 @@
 int mdwf_launch_hop_D(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
-int mdwf_launch_hop4_S(int, int, int, int, const HopArgs &, cudaStream_t);
-int mdwf_launch_hop4_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_sdense_mma(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
@@ -27,11 +25,6 @@ int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const v
 
 int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
 {
-    if (a.kver >= 4 && p != PREC_D) {        // v4 family (staged neighbours); -1 = not covered, fall back to v3
-        const int rc = (p == PREC_S) ? mdwf_launch_hop4_S(dag, pre, post, own, a, st)
-                                     : mdwf_launch_hop4_H(dag, pre, post, own, a, st);
-        if (rc != -1) return rc;
-    }
     if (a.kver >= 3 && p != PREC_D) {        // v3 family (fp32 arithmetic); -1 = not covered, fall back to v2
         const int rc = (p == PREC_S) ? mdwf_launch_hop3_S(dag, pre, post, own, a, st)
                                      : mdwf_launch_hop3_H(dag, pre, post, own, a, st);
@@ -70,7 +63,8 @@ struct mdwf_ctx {
     double delta = 0.1;
     int max_update_interval = 0;
     int use_bp = 1;          // 16-bit Krylov vectors: let the CG update write B p for K1 (option "bp_stream")
-    int kver = 3;            // kernel family for fp32 arithmetic: 3 = hop3_kernels.cuh, 2 = hop_kernels.cuh
+    int kver = 3;            // kernel family for fp32 arithmetic: 3 = hop3_kernels.cuh (link tile by TMA, spinors through registers),
+                             // 4 = the same with the t+- neighbour groups staged by TMA too, 2 = hop_kernels.cuh
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
@@ -255,8 +249,9 @@ static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const Spinor
     a.in = in.v; a.in_norm = in.norm;
     a.own = own ? own->v : nullptr; a.own_norm = own ? own->norm : nullptr;
     a.out = out.v; a.out_norm = out.norm;
-    a.gauge_same = c->gauge[p][parity_out];
-    a.gauge_other = c->gauge[p][1 - parity_out];
+    a.gauge = c->gauge[p][parity_out];
+    a.dLxh = mdwf_fastdiv((unsigned)(c->L[0] / 2)); a.dLy = mdwf_fastdiv((unsigned)c->L[1]); a.dLz = mdwf_fastdiv((unsigned)c->L[2]);
+    a.dnb = mdwf_fastdiv((unsigned)a.sweep_nb); a.dchunk = mdwf_fastdiv((unsigned)(a.sweep_nb * c->L[3]));
     a.recon = c->recon;
     a.mf = c->mf;
     return a;
@@ -498,7 +493,10 @@ int mdwf_load_gauge(mdwf_ctx *c, const void *U_dev, int real_bytes)
     }
     for (int p = 0; p < 3; p++)
         for (int q = 0; q < 2; q++) {
-            if (!c->gauge[p][q]) CUDA_OK(c, cudaMalloc(&c->gauge[p][q], mdwf_gauge_bytes((Prec)p, c->Vh, recon)));
+            if (!c->gauge[p][q]) {
+                CUDA_OK(c, cudaMalloc(&c->gauge[p][q], mdwf_gauge_bytes((Prec)p, c->Vh, recon)));
+                CUDA_OK(c, cudaMemsetAsync(c->gauge[p][q], 0, mdwf_gauge_bytes((Prec)p, c->Vh, recon), c->st));   // padding lanes of a ragged last group
+            }
             CUDA_OK(c, mdwf_launch_gauge_in((Prec)p, U_dev, real_bytes, c->gauge[p][q], c->L, q, recon, c->st));
             c->launches += 1;
         }

@@ -8,7 +8,8 @@
 // contiguous bytes per instruction and the chunk index becomes an immediate offset in the load.
 // All L5 slices of a 32-site group are contiguous (L5*NV*512 B), which keeps the s-neighbourhood of a
 // site group in a few DRAM pages.  The 16-bit format adds norm[(g*L5 + s)*32 + lane] (fp32 scale).
-// Gauge links of the sites of one parity: link[ ((g*4 + mu)*NK + k)*32 + lane ], one complex per chunk.
+// Gauge links of the sites of one parity: link[ ((g*8 + d)*NK + k)*32 + lane ], one complex per chunk; d = mu is
+// U_mu(x), d = 4 + mu is U_mu(x - mu)^dagger pulled back to x (the 8 links of a 32-site group are one slab).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -120,14 +121,15 @@ MDWF_DEV void gunpack(const short2 c, float *r)
     r[0] = fixed_to_float((unsigned short)c.x) * (1.0f / MDWF_FIXED_MAX);
     r[1] = fixed_to_float((unsigned short)c.y) * (1.0f / MDWF_FIXED_MAX);
 }
-// U[2*(row*3+col)+ri]; with recon == 12 the third row is conj(row0 x row1).
+// U[2*(row*3+col)+ri] of direction d (0-3 forward, 4-7 backward, already daggered) at site cb; with recon == 12 the
+// third row is conj(row0 x row1).
 template <class P>
-MDWF_DEV void load_link(const void *gbase, int mu, long cb, int recon, typename P::R *U)
+MDWF_DEV void load_link(const void *gbase, int d, long cb, int recon, typename P::R *U)
 {
     using G = typename P::G;
     using R = typename P::R;
     const int NK = recon >> 1;
-    const G *p = reinterpret_cast<const G *>(gbase) + ((((cb >> 5) * 4 + mu) * NK) << 5) + (cb & 31);
+    const G *p = reinterpret_cast<const G *>(gbase) + ((((cb >> 5) * 8 + d) * NK) << 5) + (cb & 31);
 #pragma unroll
     for (int k = 0; k < 6; k++) gunpack(__ldg(p + 32 * k), U + 2 * k);
     if (recon == 18) {

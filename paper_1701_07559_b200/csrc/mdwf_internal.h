@@ -4,8 +4,8 @@
 //   parity spinor, precision P:  chunk[((g*L5 + s)*NV + j)*32 + lane], chunk = double2 (fp64, NV=12, one
 //                                complex), float4 (fp32, NV=6, two complex) or short4 (16-bit fixed point,
 //                                NV=6) with one float scale norm[(g*L5 + s)*32 + lane] per 5D site.
-//   gauge, per parity p of the site the link starts from: link[((g*4 + mu)*NK + k)*32 + lane], one complex
-//                                per chunk (double2 / float2 / short2), NK = 9 (18 reals) or 6 (12 reals).
+//   gauge, per parity p of the site x: link[((g*8 + d)*NK + k)*32 + lane], one complex per chunk (double2 / float2 /
+//                                short2), NK = 9 (18 reals) or 6 (12 reals); d = mu: U_mu(x), d = 4 + mu: U_mu(x-mu)^dagger.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -20,6 +20,13 @@
 #ifndef MDWF_H3_WARPS_H
 #define MDWF_H3_WARPS_H 12
 #endif
+// neighbour groups staged by the TMA engine in the v3 kernels (0, 2 = t+-, 4 = z+- and t+-), per storage format
+#ifndef MDWF_H3_NST_S
+#define MDWF_H3_NST_S 2
+#endif
+#ifndef MDWF_H3_NST_H
+#define MDWF_H3_NST_H 2
+#endif
 static inline int mdwf_h3_slices(int L5) { return L5 == 12 ? MDWF_H3_S12 : 2; }
 
 enum Prec { PREC_D = 0, PREC_S = 1, PREC_H = 2 };
@@ -29,8 +36,25 @@ struct SpinorBuf {       // one single-parity 5D vector in a device layout
     float *norm = nullptr;   // 16-bit format only
 };
 
+// n / d for 0 <= n < 2^31 as  __umulhi(n, m) >> s  (m = 0: d == 1)
+struct FastDiv {
+    unsigned m, s, d;
+};
+static inline FastDiv mdwf_fastdiv(unsigned d)
+{
+    FastDiv f;
+    f.d = d;
+    if (d <= 1) { f.m = 0; f.s = 0; return f; }
+    unsigned sh = 0;
+    while ((1ull << sh) < d) sh++;                       // 2^(sh-1) < d <= 2^sh
+    f.m = (unsigned)((1ull << (31 + sh)) / d + 1);
+    f.s = sh - 1;
+    return f;
+}
+
 struct HopArgs {
     int L[4];
+    FastDiv dLxh, dLy, dLz, dnb, dchunk;   // Lx/2, Ly, Lz, sweep_nb, sweep_nb * Lt
     int L5;
     int Vh;
     int parity_out;          // parity of the sites this launch writes
@@ -42,8 +66,7 @@ struct HopArgs {
     const float *own_norm;
     void *out;
     float *out_norm;
-    const void *gauge_same;  // links starting at sites of parity_out      (forward hops)
-    const void *gauge_other; // links starting at sites of the other parity (backward hops)
+    const void *gauge;       // link tiles of the sites of parity_out: 8 directions per site (4 forward, 4 backward pulled back)
     int recon;               // 18 or 12
     double coef_hop;         // multiplies the hop sum
     double pre_d, pre_o;     // PRE = 1: input is (pre_d + pre_o Lambda) psi        (B on load)
@@ -53,7 +76,7 @@ struct HopArgs {
     double *partial;         // v3 kernels: if non-null, ||out||^2 partial sums, one per block (fused norm, S7)
     const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
     // POST = 1 in the v3 kernels (hop3_kernels.cuh): coef_hop * B A^{-1} as a blocked recurrence
-    int kver;                // host side: kernel family requested (2 or 3)
+    int kver;                // host side: kernel family requested (2: hop_kernels.cuh, 3: hop3 all-LDG, 4: hop3 with TMA-staged z/t neighbours)
     int r_ok;                // 1 when the recurrence form is usable (|kappa| < 1)
     float r_nk;              // -kappa = -beta/alpha
     float r_cpow;            // (-kappa)^S, S = slices per thread
