@@ -241,38 +241,80 @@ MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
 // PRE = 1 applies (1 + f Lambda) to the neighbour on load: upper spins add f * (slice s-1), lower spins
 // f * (slice s+1), wall factor -m_f at the wrap.  The window slides over the S slices (one half-spinor of
 // halo on each side), so only one full slice and two half slices are live at a time.
-// gb / nb: chunk 0 of slice 0 and scale of slice 0 of this thread's neighbour site; slice s is at gb + s*32*NV, nb + 32 s,
-// in global memory (G = true) as well as in a staged group (G = false), which keeps the [s][chunk][lane] layout.
+// The neighbour's slices are read through a source object: SrcMem = global memory (G = true, read-only path) or a group
+// staged in shared memory (G = false), which keeps the [s][chunk][lane] layout; SrcReg = raw chunks loaded into
+// registers ahead of their use (the first direction of a block, whose loads are issued before the link tile is waited
+// for).  Window slice k = 0..S-1 is slice s0 + k; k = -1 / k = S are the halo slices of the B-on-load stencil.
 template <class P, bool G> MDWF_DEV float ld_scale(const float *np)
 {
     if (!P::HALF) return 1.0f;
     return ldx<G>(np) * (1.0f / MDWF_FIXED_MAX);
 }
-template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR, bool G>
-MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const typename P::V *gb, const float *nb, float bsign,
-                        c2 (*acc)[12])
+template <class P, int S, bool G> struct SrcMem {
+    const typename P::V *gb;      // chunk 0 of slice 0 of this thread's neighbour site
+    const float *nb;              // scale of slice 0 (16-bit storage)
+    int s0, sm, sp;               // first slice of the window, slice below (wrapped), slice above (wrapped)
+    MDWF_DEV int slice(int k) const { return k < 0 ? sm : (k >= S ? sp : s0 + k); }
+    MDWF_DEV typename P::V chunk(int k, int j) const { return ldx<G>(gb + slice(k) * (32 * P::NV) + 32 * j); }
+    MDWF_DEV float scale(int k) const { return ld_scale<P, G>(nb + 32 * slice(k)); }
+};
+template <class P, int PRE, int S> struct SrcReg {
+    typename P::V q[S][6], up[3], lo[3];
+    float sc[S], scu, scl;
+    template <bool G> MDWF_DEV void load(const SrcMem<P, S, G> &m)
+    {
+#pragma unroll
+        for (int k = 0; k < S; k++) {
+#pragma unroll
+            for (int j = 0; j < 6; j++) q[k][j] = m.chunk(k, j);
+            sc[k] = m.scale(k);
+        }
+        if (PRE) {
+#pragma unroll
+            for (int j = 0; j < 3; j++) { up[j] = m.chunk(-1, j); lo[j] = m.chunk(S, 3 + j); }
+            scu = m.scale(-1);
+            scl = m.scale(S);
+        }
+    }
+    MDWF_DEV typename P::V chunk(int k, int j) const { return k < 0 ? up[j] : (k >= S ? lo[j - 3] : q[k][j]); }
+    MDWF_DEV float scale(int k) const { return k < 0 ? scu : (k >= S ? scl : sc[k]); }
+};
+// chunk -> two complex numbers; SCALED = false leaves the 16-bit integers unscaled (the scale then goes into the
+// reconstruction weight: the hop is linear)
+template <bool SCALED> MDWF_DEV void unp(const float4 q, float, c2 &x, c2 &y) { x = mk(q.x, q.y); y = mk(q.z, q.w); }
+template <bool SCALED> MDWF_DEV void unp(const short4 q, float sc, c2 &x, c2 &y)
 {
-    using V = typename P::V;
+    const uint2 w = *reinterpret_cast<const uint2 *>(&q);       // the two 32-bit words as loaded: no repacking
+    const unsigned w0 = w.x, w1 = w.y;
+    if (SCALED) { x = cvt_pair(w0, dup(sc)); y = cvt_pair(w1, dup(sc)); }
+    else { x = cvt_raw(w0); y = cvt_raw(w1); }
+}
+// complexes [2*J0, 2*J0 + 2*NJ) of window slice k into v[0 .. 2*NJ)
+template <bool SCALED, int J0, int NJ, class SRC> MDWF_DEV void take(const SRC &src, int k, float sc, c2 *v)
+{
+#pragma unroll
+    for (int j = 0; j < NJ; j++) unp<SCALED>(src.chunk(k, J0 + j), sc, v[2 * j], v[2 * j + 1]);
+}
+
+template <class P, int MU, bool FWD, int DAG, int PRE, int S, bool TDIR, class SRC>
+MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const SRC &src, float bsign, c2 (*acc)[12])
+{
     constexpr int SGN = (FWD ? 1 : -1) * (DAG ? -1 : 1);
     Link U;
     load_link3(sl, U);
-
-    constexpr long SL = 32 * P::NV;
-    const V *p0 = gb + s0 * SL;
-    const float *n0 = nb + 32 * s0;
 
     if (PRE == 0) {
 #pragma unroll
         for (int k = 0; k < S; k++) {
             c2 v[12], h[6], chi[6];
             if constexpr (P::HALF) {
-                const float sck = ld_scale<P, G>(n0 + 32 * k);
-                Ld<P>::template raw<12, G>(p0 + k * SL, v);
+                const float sck = src.scale(k);
+                take<false, 0, 6>(src, k, 1.f, v);
                 project3<MU, SGN>(v, h);
                 su3_mul3(U, h, chi);
                 recon3<MU, SGN, true>(chi, TDIR ? bsign * sck : sck, acc[k]);
             } else {
-                Ld<P>::template chunks<12, G>(p0 + k * SL, 1.0f, v);
+                take<true, 0, 6>(src, k, 1.f, v);
                 project3<MU, SGN>(v, h);
                 su3_mul3(U, h, chi);
                 recon3<MU, SGN, TDIR>(chi, bsign, acc[k]);
@@ -280,18 +322,13 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const
         }
     } else {
         const float f = (float)(a.pre_o / a.pre_d), fw = (float)(-a.mf * a.pre_o / a.pre_d);
-        const int sm = (s0 == 0) ? L5 - 1 : s0 - 1;
-        const int sp = (s0 + S >= L5) ? 0 : s0 + S;
         c2 prev_up[6], cur[12], nxt[12];
-        Ld<P>::template chunks<6, G>(gb + sm * SL, ld_scale<P, G>(nb + 32 * sm), prev_up);
-        Ld<P>::template chunks<12, G>(p0, ld_scale<P, G>(n0), cur);
+        take<true, 0, 3>(src, -1, src.scale(-1), prev_up);
+        take<true, 0, 6>(src, 0, src.scale(0), cur);
 #pragma unroll
         for (int k = 0; k < S; k++) {
-            if (k < S - 1) {
-                Ld<P>::template chunks<12, G>(p0 + (k + 1) * SL, ld_scale<P, G>(n0 + 32 * (k + 1)), nxt);
-            } else {
-                Ld<P>::template chunks<6, G>(gb + sp * SL + 32 * (P::NV / 2), ld_scale<P, G>(nb + 32 * sp), nxt + 6);
-            }
+            if (k < S - 1) take<true, 0, 6>(src, k + 1, src.scale(k + 1), nxt);
+            else take<true, 3, 3>(src, S, src.scale(S), nxt + 6);
             const c2 fu = dup((s0 + k == 0) ? fw : f);
             const c2 fl = dup((s0 + k == L5 - 1) ? fw : f);
             c2 w[12], h[6], chi[6];
@@ -650,6 +687,14 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
     const float btp = (t == Lt - 1) ? -1.f : 1.f;               // antiperiodic in t
     const float btm = (t == 0) ? -1.f : 1.f;
 
+    // the loads of the first direction (x+) go out before the link tile is waited for
+    const V *gin = reinterpret_cast<const V *>(a.in);
+    const int sm = (s0 == 0) ? L5 - 1 : s0 - 1, sp = (s0 + S >= L5) ? 0 : s0 + S;
+    // (fp32 storage only: at the 168 registers of the 16-bit kernels the early loads spill and cost more than they hide)
+    constexpr bool EARLY = !P::HALF;
+    SrcReg<P, PRE, EARLY ? S : 1> first;
+    if (EARLY && active) first.load(SrcMem<P, EARLY ? S : 1, true>{gin + sp_off(L5, NV, nb[0], 0), a.in_norm + sp_noff(L5, nb[0], 0), s0, sm, sp});
+
     // the link tile has landed (its latency ran under the index arithmetic above): warp d mod NSG completes direction d
     __syncthreads();                                             // barrier initialisation visible to every thread
     mbar_wait(&bar[0], 0);
@@ -659,18 +704,18 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
     __syncthreads();
 
     if (active) {
-        const V *gin = reinterpret_cast<const V *>(a.in);
-        // neighbour in global memory: chunk 0 of slice 0 / scale of slice 0 of site nb[d]
+        // neighbour in global memory: chunk 0 of slice 0 / scale of slice 0 of site nb[d];  d = FWD ? MU : 4 + MU
 #define MDWF_GDIR(MU, FWD, TD, d, bs) \
-        hop_dir3<P, MU, FWD, DAG, PRE, S, TD, true>(a, L5, s0, sL + (d) * 288 + lane, gin + sp_off(L5, NV, nb[d], 0), \
-                                                    a.in_norm + sp_noff(L5, nb[d], 0), bs, acc)   /* d = FWD ? MU : 4 + MU */
+        hop_dir3<P, MU, FWD, DAG, PRE, S, TD>(a, L5, s0, sL + (d) * 288 + lane, \
+            SrcMem<P, S, true>{gin + sp_off(L5, NV, nb[d], 0), a.in_norm + sp_noff(L5, nb[d], 0), s0, sm, sp}, bs, acc)
         // neighbour group staged in slot k: same lane
 #define MDWF_SDIR(MU, FWD, TD, d, bs, k) \
         do { mbar_wait(&bar[1 + (k)], 0); \
-             hop_dir3<P, MU, FWD, DAG, PRE, S, TD, false>(a, L5, s0, sL + (d) * 288 + lane, \
-                 reinterpret_cast<const V *>(smem_raw3 + (k) * SLOT_BYTES) + lane, \
-                 reinterpret_cast<const float *>(smem_raw3 + (k) * SLOT_BYTES + BUF_BYTES) + lane, bs, acc); } while (0)
-        MDWF_GDIR(0, true, false, 0, 1.f);
+             hop_dir3<P, MU, FWD, DAG, PRE, S, TD>(a, L5, s0, sL + (d) * 288 + lane, \
+                 SrcMem<P, S, false>{reinterpret_cast<const V *>(smem_raw3 + (k) * SLOT_BYTES) + lane, \
+                                     reinterpret_cast<const float *>(smem_raw3 + (k) * SLOT_BYTES + BUF_BYTES) + lane, s0, sm, sp}, bs, acc); } while (0)
+        if constexpr (EARLY) hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, first, 1.f, acc);
+        else MDWF_GDIR(0, true, false, 0, 1.f);
         MDWF_GDIR(0, false, false, 4, 1.f);
         MDWF_GDIR(1, true, false, 1, 1.f);
         MDWF_GDIR(1, false, false, 5, 1.f);
