@@ -107,6 +107,16 @@ int mdwf_blas_norm2(mdwf_ctx *ctx, const void *x_dev, long long n, int real_byte
 int mdwf_blas_redot(mdwf_ctx *ctx, const void *x_dev, const void *y_dev, long long n, int real_bytes, double *out);
 int mdwf_blas_axpy(mdwf_ctx *ctx, double a, const void *x_dev, void *y_dev, long long n, int real_bytes);
 
+/* The 16-bit storage format of the sloppy precision as it is stored (the paper
+ * says only "double-half"): one fp32 scale m = max |component| per (site, s) and 24 unsigned 16-bit words
+ * u = round_to_nearest_even(v * (32767 / m)) + 32768, decoded as (u - 32768) * (m * (1 / 32767)) in fp32.
+ * encode: parity spinor psi[s][cb][spin][colour] (real_bytes 8 or 4) -> words_dev uint16[s][cb][24], scales_dev
+ * float[s][cb]; via_fp64 = 0 quantises the buffer with the layout kernel (the path of mdwf_apply), 1 converts it to the
+ * fp64 device layout first and quantises with the BLAS-1 copy (the path of mdwf_solve).  decode is the inverse map.
+ * Integer work: tests compare the words and scales bit for bit with a restatement of the formula. */
+int mdwf_half_encode(mdwf_ctx *ctx, const void *in_dev, int real_bytes, int via_fp64, void *words_dev, void *scales_dev);
+int mdwf_half_decode(mdwf_ctx *ctx, const void *words_dev, const void *scales_dev, void *out_dev, int real_bytes);
+
 /* Per-context counters.  Keys: "launches" (kernels launched so far), "iterations", "reliable_updates",
  * "solve_seconds" (device time of the last solve, CUDA events), "true_residual", "op_applications"
  * (Mpc + Mpc^dagger applications in the last solve, all precisions), "sloppy_applications". */

@@ -15,7 +15,8 @@ OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG = 0, 1, 2, 3, 4
 
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
-           "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates"]
+           "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
+           "mdwf_half_encode", "mdwf_half_decode"]
 
 _lib = None
 
@@ -52,6 +53,8 @@ def lib():
         L.mdwf_flops_per_site.argtypes = [P]
         L.mdwf_time_op.argtypes = [P, I, ctypes.c_char_p, I, I, ctypes.POINTER(D)]
         L.mdwf_fma_rates.argtypes = [P, ctypes.POINTER(D)]
+        L.mdwf_half_encode.argtypes = [P, P, I, I, P, P]
+        L.mdwf_half_decode.argtypes = [P, P, P, P, I]
         _lib = L
     return _lib
 
@@ -176,6 +179,22 @@ class Mdwf:
         out = (ctypes.c_double * 2)()
         _check(self.h, lib().mdwf_fma_rates(self.h, out))
         return out[0], out[1]
+
+    def half_encode(self, x, via_fp64=False):
+        """parity spinor [L5][Vh][4][3] -> (uint16 words [L5][Vh][24], fp32 scales [L5][Vh]) as the 16-bit format stores them"""
+        import torch
+        assert x.is_cuda and x.is_contiguous()
+        words = torch.empty(x.shape[0], x.shape[1], 24, dtype=torch.int16, device=x.device)
+        scales = torch.empty(x.shape[0], x.shape[1], dtype=torch.float32, device=x.device)
+        _check(self.h, lib().mdwf_half_encode(self.h, x.data_ptr(), self._rb(x), int(via_fp64), words.data_ptr(), scales.data_ptr()))
+        return words, scales
+
+    def half_decode(self, words, scales, dtype=None):
+        import torch
+        dtype = dtype or torch.complex64
+        out = torch.empty(words.shape[0], words.shape[1], 4, 3, dtype=dtype, device=words.device)
+        _check(self.h, lib().mdwf_half_decode(self.h, words.data_ptr(), scales.data_ptr(), out.data_ptr(), self._rb(out)))
+        return out
 
     def norm2(self, x):
         v = ctypes.c_double(0.0)

@@ -194,6 +194,48 @@ int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, c
 #undef C
 }
 
+// ---- the 16-bit storage format as stored: words[(s*Vh + cb)*24 + k] (offset binary), scales[s*Vh + cb] ---------------
+__global__ void half_export_kernel(const void *src, const float *src_norm, unsigned short *words, float *scales, int L5, long Vh)
+{
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)L5 * Vh) return;
+    const int s = (int)(idx / Vh);
+    const long cb = idx - (long)s * Vh;
+    const short4 *p = reinterpret_cast<const short4 *>(src) + sp_off(L5, PH::NV, cb, s);
+#pragma unroll
+    for (int j = 0; j < PH::NV; j++) {
+        const short4 q = p[32 * j];
+        words[idx * 24 + 4 * j] = (unsigned short)q.x; words[idx * 24 + 4 * j + 1] = (unsigned short)q.y;
+        words[idx * 24 + 4 * j + 2] = (unsigned short)q.z; words[idx * 24 + 4 * j + 3] = (unsigned short)q.w;
+    }
+    scales[idx] = src_norm[sp_noff(L5, cb, s)];
+}
+__global__ void half_import_kernel(const unsigned short *words, const float *scales, void *dst, float *dst_norm, int L5, long Vh)
+{
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long)L5 * Vh) return;
+    const int s = (int)(idx / Vh);
+    const long cb = idx - (long)s * Vh;
+    short4 *p = reinterpret_cast<short4 *>(dst) + sp_off(L5, PH::NV, cb, s);
+#pragma unroll
+    for (int j = 0; j < PH::NV; j++)
+        p[32 * j] = make_short4((short)words[idx * 24 + 4 * j], (short)words[idx * 24 + 4 * j + 1], (short)words[idx * 24 + 4 * j + 2],
+                                (short)words[idx * 24 + 4 * j + 3]);
+    dst_norm[sp_noff(L5, cb, s)] = scales[idx];
+}
+int mdwf_launch_half_export(const SpinorBuf &src, void *words, void *scales, int L5, int Vh, cudaStream_t st)
+{
+    const long n = (long)L5 * Vh;
+    half_export_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(src.v, src.norm, (unsigned short *)words, (float *)scales, L5, Vh);
+    return (int)cudaGetLastError();
+}
+int mdwf_launch_half_import(const void *words, const void *scales, const SpinorBuf &dst, int L5, int Vh, cudaStream_t st)
+{
+    const long n = (long)L5 * Vh;
+    half_import_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>((const unsigned short *)words, (const float *)scales, dst.v, dst.norm, L5, Vh);
+    return (int)cudaGetLastError();
+}
+
 // ---- timing inputs: hash-filled vectors ------------------------------------------------------------
 template <class P>
 __global__ void fill_kernel(void *dst, float *dst_norm, int L5, long Vh, unsigned seed)

@@ -756,6 +756,38 @@ int mdwf_solve_host(mdwf_ctx *c, const void *src_host, void *sol_host, double to
     return rc;
 }
 
+// ---- the 16-bit storage format, as stored (bit-exact tests of the quantiser) ------------------------------------------
+int mdwf_half_encode(mdwf_ctx *c, const void *in_dev, int real_bytes, int via_fp64, void *words_dev, void *scales_dev)
+{
+    if (!c || !in_dev || !words_dev || !scales_dev || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    SpinorBuf h, d;
+    TRY(get_spinor(c, "hf.h", PREC_H, &h));
+    if (via_fp64) {     // the path of the solver: fp64 device vector -> 16-bit by the BLAS-1 copy
+        TRY(get_spinor(c, "hf.d", PREC_D, &d));
+        CUDA_OK(c, mdwf_launch_parity_in(PREC_D, in_dev, real_bytes, d, c->L5, c->Vh, c->st));
+        c->launches += 1;
+        TRY(v_axpby(c, PREC_H, h, 1.0, PREC_D, d, 0.0, PREC_D, nullptr, nullptr));
+    } else {            // the path of mdwf_apply: canonical buffer -> 16-bit by the layout kernel
+        CUDA_OK(c, mdwf_launch_parity_in(PREC_H, in_dev, real_bytes, h, c->L5, c->Vh, c->st));
+        c->launches += 1;
+    }
+    CUDA_OK(c, mdwf_launch_half_export(h, words_dev, scales_dev, c->L5, c->Vh, c->st));
+    c->launches += 1;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
+}
+int mdwf_half_decode(mdwf_ctx *c, const void *words_dev, const void *scales_dev, void *out_dev, int real_bytes)
+{
+    if (!c || !out_dev || !words_dev || !scales_dev || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    SpinorBuf h;
+    TRY(get_spinor(c, "hf.h", PREC_H, &h));
+    CUDA_OK(c, mdwf_launch_half_import(words_dev, scales_dev, h, c->L5, c->Vh, c->st));
+    CUDA_OK(c, mdwf_launch_parity_out(PREC_H, h, out_dev, real_bytes, c->L5, c->Vh, c->st));
+    c->launches += 2;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
+}
+
 // ---- S7 entry points on flat arrays ---------------------------------------------------------------------
 int mdwf_blas_norm2(mdwf_ctx *c, const void *x, long long n, int real_bytes, double *out)
 {

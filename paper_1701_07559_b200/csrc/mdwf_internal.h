@@ -131,6 +131,10 @@ int mdwf_launch_full_out(Prec p, const SpinorBuf &src, void *canon, int real_byt
 int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, const int *L, int parity, int recon,
                          cudaStream_t st);
 
+// the 16-bit format as stored, in canonical order: words[(s*Vh + cb)*24 + k] (uint16, offset binary), scales[s*Vh + cb]
+int mdwf_launch_half_export(const SpinorBuf &src, void *words, void *scales, int L5, int Vh, cudaStream_t st);
+int mdwf_launch_half_import(const void *words, const void *scales, const SpinorBuf &dst, int L5, int Vh, cudaStream_t st);
+
 // deterministic pseudo-random fill in [-1,1] (timing inputs only)
 int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st);
 

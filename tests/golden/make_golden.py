@@ -28,7 +28,9 @@ def compute():
                     ("Mpcdag b_o", orc.Mpcdag(orc.parity_part(b, 1)))):
         f = v.ravel()
         rows.append((name + " norm2", float(np.vdot(f, f).real), 0.0))
-        for k in (0, 7, f.size // 2 + 5, f.size - 1):
+        # sample non-zero entries only (the single-parity results vanish on every even site): first, 8th, middle, last
+        nz = np.flatnonzero(f)
+        for k in (nz[0], nz[7], nz[nz.size // 2 + 5], nz[-1]):
             rows.append((f"{name} [{k}]", float(f[k].real), float(f[k].imag)))
     return rows
 

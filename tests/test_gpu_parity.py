@@ -1,7 +1,10 @@
 """Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
 seeded inputs.  Tolerances are BASELINE.json's: rel. L2 <= 1e-12 (fp64), <= 1e-5 (fp32); solves reach an
 ORACLE-recomputed true residual <= 1e-10.  The 16-bit operator has no tolerance in the paper or in
-north_star; DESIGN.md section 5 derives 2e-3 from the 15-bit mantissa of the fixed-point format.
+north_star; DESIGN.md section 4 derives 2e-4 for it: every stored component carries an error <= m/65534 (m = the
+largest component of its (site, s) spinor; tests/test_gpu_half_format.py), i.e. <= 2^-16 sqrt(24) / ||v_site||-relative
+~ 1e-5 per vector for Gaussian data, and one Mpc quantises three vectors (input, the even-site intermediate, output)
+and reads near-unitary 16-bit links (1.5e-5 each): ~4e-5 in relative L2, 1-4e-5 measured; the bound asserted is 5x that.
 """
 import numpy as np
 import pytest
@@ -24,7 +27,7 @@ CASES = {
     "shamir": ((4, 4, 2, 2), 8, 1.8, 1.0, 0.0, 0.0, 0.3, 14),          # c5 = 0 (B = 1, kappa = -1/alpha), m_f = 0
     "kappa1": ((4, 4, 2, 2), 8, 1.3, 0.001, 0.0, 0.05, 0.3, 15),       # |kappa| = 0.997: recurrence refused, dense table used
 }
-TOL = {"fp64": 1e-12, "fp32": 1e-5, "half": 2e-3}
+TOL = {"fp64": 1e-12, "fp32": 1e-5, "half": 2e-4}
 
 
 def setup(name, recon="18"):
