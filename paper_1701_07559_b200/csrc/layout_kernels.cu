@@ -67,8 +67,10 @@ MDWF_DEV float2 gpack(double re, double im, float2 *) { return make_float2((floa
 MDWF_DEV short2 gpack(double re, double im, short2 *)
 {
     // offset binary, like the spinors (mdwf_device.cuh)
-    return make_short2((short)(unsigned short)(__double2int_rn(re * (double)MDWF_FIXED_MAX) + 32768),
-                       (short)(unsigned short)(__double2int_rn(im * (double)MDWF_FIXED_MAX) + 32768));
+    // clamped: a component above 1 (a non-unitary field) saturates instead of wrapping
+    const int qr = max(-32767, min(32767, __double2int_rn(re * (double)MDWF_FIXED_MAX)));
+    const int qi = max(-32767, min(32767, __double2int_rn(im * (double)MDWF_FIXED_MAX)));
+    return make_short2((short)(unsigned short)(qr + 32768), (short)(unsigned short)(qi + 32768));
 }
 
 // Link tile of a site x of the given parity, 8 directions d:

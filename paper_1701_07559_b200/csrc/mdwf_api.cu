@@ -300,6 +300,11 @@ static bool fused_norm_available(const mdwf_ctx *c, Prec p)
 {
     return p != PREC_D && c->kver >= 3 && (c->L5 == 8 || c->L5 == 12 || c->L5 == 16);
 }
+// K1 reading a precomputed B p exists only in the recurrence (v3) family: |kappa| < 0.98, see fill_recurrence
+static bool bp_stream_available(const mdwf_ctx *c, Prec p)
+{
+    return fused_norm_available(c, p) && std::fabs(c->beta / c->alpha) < 0.98;
+}
 static int finish_norm(mdwf_ctx *c, Prec p, const SpinorBuf &out, bool fused, double *norm2_out)
 {
     if (!norm2_out) return MDWF_OK;
@@ -487,7 +492,9 @@ int mdwf_load_gauge(mdwf_ctx *c, const void *U_dev, int real_bytes)
     int ndev = 0;
     CUDA_OK(c, cudaGetDeviceCount(&ndev));
     const int recon = c->recon_opt;
-    if (c->gauge_loaded && recon != c->recon) {
+    const bool had = c->gauge_loaded;
+    c->gauge_loaded = false;                 // true again only after every step below has succeeded
+    if (had && recon != c->recon) {
         for (int p = 0; p < 3; p++)
             for (int q = 0; q < 2; q++) { cudaFree(c->gauge[p][q]); c->gauge[p][q] = nullptr; }
     }
@@ -597,7 +604,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     TRY(get_spinor(c, "sv.ts", ps, &ts));
     TRY(get_spinor(c, "sv.xlo", pxl, &xlo));
     // 16-bit Krylov vectors: the CG update also writes B p, and p is double-buffered
-    const bool use_bp = (ps == PREC_H) && fused_norm_available(c, ps) && c->use_bp;
+    const bool use_bp = (ps == PREC_H) && bp_stream_available(c, ps) && c->use_bp;
     SpinorBuf p2, bpv;
     if (use_bp) { TRY(get_spinor(c, "sv.p2", ps, &p2)); TRY(get_spinor(c, "sv.bp", ps, &bpv)); }
 
@@ -715,7 +722,11 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     c->true_residual = tr;
     if (iters_out) *iters_out = k;
     if (true_res_out) *true_res_out = tr;
-    if (!(tr <= tol * 1.0000001) && !converged) { c->err = "CG did not converge within maxiter"; return MDWF_ENOCONV; }
+    if (!(tr <= tol * 1.001)) {              // the header's contract: tol is the target for ||src - D x|| / ||src||
+        c->err = converged ? "CG converged on the Schur system but the recomputed full residual exceeds tol"
+                           : "CG did not converge within maxiter";
+        return MDWF_ENOCONV;
+    }
     return MDWF_OK;
 }
 
@@ -726,8 +737,8 @@ int mdwf_solve(mdwf_ctx *c, const void *src_dev, void *sol_dev, double tol, int 
     if (!src_dev || !sol_dev || src_dev == sol_dev || !(tol > 0.0) || maxiter < 0) { c->err = "mdwf_solve: bad argument"; return MDWF_EARG; }
     cudaEvent_t e0, e1;
     CUDA_OK(c, cudaEventCreate(&e0));
-    CUDA_OK(c, cudaEventCreate(&e1));
-    CUDA_OK(c, cudaEventRecord(e0, c->st));
+    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); c->err = "cudaEventCreate"; return MDWF_ECUDA; }
+    if (cudaEventRecord(e0, c->st) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); c->err = "cudaEventRecord"; return MDWF_ECUDA; }
     const int rc = solve_device(c, src_dev, sol_dev, tol, maxiter, iters_out, true_res_out);
     cudaEventRecord(e1, c->st);
     cudaEventSynchronize(e1);
@@ -813,7 +824,7 @@ int mdwf_blas_axpy(mdwf_ctx *c, double a, const void *x, void *y, long long n, i
     return MDWF_OK;
 }
 
-int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4)
+static int time_op_events(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4, cudaEvent_t e0, cudaEvent_t e1)
 {
     TRY(check_ready(c));
     if (!precision || !out4 || reps < 1 || warmup < 0 || (op != MDWF_OP_MPC && op != MDWF_OP_MPCDAG)) return MDWF_EARG;
@@ -828,15 +839,12 @@ int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmu
     CUDA_OK(c, mdwf_launch_fill(p, a, c->L5, c->Vh, 12345u, c->st));
     CUDA_OK(c, mdwf_launch_fill(p, t, c->L5, c->Vh, 999u, c->st));
     c->launches += 2;
-    cudaEvent_t e0, e1;
-    CUDA_OK(c, cudaEventCreate(&e0));
-    CUDA_OK(c, cudaEventCreate(&e1));
     const double l0 = c->launches;
     for (int phase = 0; phase < 3; phase++) {     // 0: K1 + K2 back to back, 1: K1 alone, 2: K2 alone
         for (int it = -warmup; it < reps; it++) {
             if (it == 0) CUDA_OK(c, cudaEventRecord(e0, c->st));
             // 16-bit Mpc: time the K1 the CG really launches (it reads the B p stream of the fused update)
-            const bool k1b = (op == MDWF_OP_MPC) && p == PREC_H && c->use_bp && fused_norm_available(c, p);
+            const bool k1b = (op == MDWF_OP_MPC) && p == PREC_H && c->use_bp && bp_stream_available(c, p);
             if (phase != 2) TRY(op == MDWF_OP_MPC ? (k1b ? op_Mpc_k1_from_B(c, p, a, t) : op_Mpc_k1(c, p, a, t)) : op_Mpcdag_k1(c, p, a, t));
             if (phase != 1) TRY(op == MDWF_OP_MPC ? op_Mpc_k2(c, p, a, t, b) : op_Mpcdag_k2(c, p, a, t, b));
         }
@@ -847,9 +855,18 @@ int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmu
         out4[phase] = (double)ms / reps;
     }
     out4[3] = c->launches - l0;
+    return MDWF_OK;
+}
+int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4)
+{
+    cudaEvent_t e0, e1;
+    if (!c) return MDWF_EARG;
+    CUDA_OK(c, cudaEventCreate(&e0));
+    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); c->err = "cudaEventCreate"; return MDWF_ECUDA; }
+    const int rc = time_op_events(c, op, precision, reps, warmup, out4, e0, e1);   // events are released on every path
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    return MDWF_OK;
+    return rc;
 }
 
 int mdwf_fma_rates(mdwf_ctx *c, double *tfma2)

@@ -121,9 +121,10 @@ def test_solve_true_residual_by_oracle(name, ladder):
     m.close()
 
 
-@pytest.mark.parametrize("name", ["l5_16", "l5_24", "lx32"])
+@pytest.mark.parametrize("name", ["l5_16", "l5_24", "lx32", "kappa1", "shamir"])
 def test_solve_other_L5(name):
-    """L5 = 16 (four k-blocks of the tensor-core A^-1), L5 = 24 (FMA fall-back), Lx = 32 with L5 = 12"""
+    """L5 = 16 (four k-blocks of the tensor-core A^-1), L5 = 24 (FMA fall-back), Lx = 32 with L5 = 12; |kappa| -> 1 (the
+    recurrence kernels refuse: no B p stream, dense-table K1) and c5 = 0 through the 16-bit ladder"""
     orc, m, b = setup(name)
     m.set_option("ladder", "dsh")
     sol, iters, tr, rc = m.solve(torch.from_numpy(b).cuda(), tol=1e-10, maxiter=5000)
