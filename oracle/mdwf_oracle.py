@@ -24,6 +24,12 @@ lattice or on a handful of sampled sites (Mpc_at_sites).
 Flop convention (D10), used wherever a rate is quoted: F_Mpc(L5) = 2880 + 48 L5 per odd
 5D site per application of Mpc or Mpc^+.
 
+SURVEY.md 8(f) rows, at the end of the class (each with its own pin in tests/test_oracle_pins3.py):
+  NEXT-1  Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B = A^{-1} Mpc, its adjoint and the solve through it
+          ("symmetric" preconditioning, PAPER.md:352,365)
+  NEXT-3  4D <-> 5D maps around the solve (Eq. (5)): wall source and D_- lift of a 4D source,
+          wall projection q = P- psi_0 + P+ psi_{L5-1}, midpoint field
+
 Pins: tests/test_oracle_pins.py (P1-P9 of SURVEY.md 8(c)).  Unpinned: nothing in this file;
 the mixed-precision ladder lives only in the CUDA path and is "parity unpinned" beyond the
 true residual.
@@ -313,3 +319,99 @@ class MdwfOracle:
     def true_residual(self, b, x):
         r = b - self.D(x)
         return float(np.sqrt(self.redot(r, r, self.sites_all) / self.redot(b, b, self.sites_all)))
+
+    # =====================================================================================================
+    # 4D <-> 5D maps (Eq. (5), defines the physical quark field q(x)
+    # on the walls and the midpoint field of the residual-mass ratio).  4D fields are eta[t][z][y][x][4][3].
+    # Readings (N1-N3): chirality convention of D5 (P- lives on s = 0, P+ on s = L5-1 for q);
+    # the source is injected on the opposite chiralities and lifted with D_- = c5 D_W - 1.
+    # =====================================================================================================
+    def _P(self, v, sign):
+        """P+ (sign = +1) or P- (sign = -1) = (1 +- gamma5)/2 with gamma5 = diag(+,+,-,-): keeps spins 0,1 or 2,3."""
+        out = np.zeros_like(v)
+        if sign > 0:
+            out[..., 0:2, :] = v[..., 0:2, :]
+        else:
+            out[..., 2:4, :] = v[..., 2:4, :]
+        return out
+
+    def wall_source(self, eta):
+        """b(x,s) = delta_{s,0} P+ eta(x) + delta_{s,L5-1} P- eta(x)."""
+        b = self.zeros()
+        b[0] += self._P(eta, +1)
+        b[self.L5 - 1] += self._P(eta, -1)
+        return b
+
+    def Dminus(self, v):
+        """D_- v = (c5 D_W - 1) v, slice by slice (D6)."""
+        return self.c5 * self.DW(v) - v
+
+    def lift(self, eta):
+        """5D source of the physical 4D propagator: D_- applied to the wall source."""
+        return self.Dminus(self.wall_source(eta))
+
+    def wall_project(self, psi):
+        """q(x) = P- psi(x,0) + P+ psi(x,L5-1)   (the quark field of Eq. (5))."""
+        return self._P(psi[0], -1) + self._P(psi[self.L5 - 1], +1)
+
+    def midpoint(self, psi):
+        """Q(x) = P- psi(x,L5/2) + P+ psi(x,L5/2-1): the wall fields moved to the middle of the fifth dimension."""
+        h = self.L5 // 2
+        return self._P(psi[h], -1) + self._P(psi[h - 1], +1)
+
+    # =====================================================================================================
+    # SURVEY.md 8(f) NEXT-1: symmetric even-odd preconditioning (PAPER.md:352,365).
+    #   Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B          (D7, last line)
+    #   Mpc_sym^+ = 1 - (1/4) B^+ H'_oe A^{-+} B^+ H'_eo A^{-+}
+    # Schur system: Mpc_sym x_o = A^{-1} b'_o with the same b' and the same reconstruction as D8.
+    # =====================================================================================================
+    def Mpc_sym(self, v_o):
+        so, se = self.sites_odd, self.sites_even
+        t1 = self.B(v_o, so)                        # B v_o
+        t2 = self.hop(t1, se)                       # H_eo B v_o
+        t3 = self.Ainv(t2, se)                      # A^{-1} H_eo B v_o
+        t4 = self.B(t3, se)                         # B A^{-1} H_eo B v_o
+        t5 = self.hop(t4, so)                       # H_oe B A^{-1} H_eo B v_o
+        t6 = self.Ainv(t5, so)                      # A^{-1} H_oe B A^{-1} H_eo B v_o
+        return self.axpby(1.0, v_o, -0.25, t6, so)
+
+    def Mpc_sym_dag(self, v_o):
+        so, se = self.sites_odd, self.sites_even
+        t0 = self.Ainv(v_o, so, dagger=True)        # A^{-+} v_o
+        t1 = self.hop(t0, se, dagger=True)          # H'_eo ...
+        t2 = self.B(t1, se, dagger=True)            # B^+ ...
+        t3 = self.Ainv(t2, se, dagger=True)         # A^{-+} ...
+        t4 = self.hop(t3, so, dagger=True)          # H'_oe ...
+        t5 = self.B(t4, so, dagger=True)            # B^+ ...
+        return self.axpby(1.0, v_o, -0.25, t5, so)
+
+    def cgls_op(self, M, Mdag, rhs, tol_abs, maxiter):
+        """D9 for a general operator pair on odd sites; stops on ||rho|| <= tol_abs.  Returns x, iterations."""
+        so = self.sites_odd
+        x = self.zeros()
+        rho = rhs.copy()
+        g = Mdag(rho)
+        p = g.copy()
+        gam = self.redot(g, g, so)
+        k = 0
+        while k < maxiter and np.sqrt(self.redot(rho, rho, so)) > tol_abs:
+            q = M(p)
+            a = gam / self.redot(q, q, so)
+            x += a * p
+            rho -= a * q
+            k += 1
+            g = Mdag(rho)
+            gam_new = self.redot(g, g, so)
+            p = g + (gam_new / gam) * p
+            gam = gam_new
+        return x, k
+
+    def solve_sym(self, b, tol=1e-10, maxiter=10000):
+        """x = D^{-1} b through the symmetric Schur system; returns x, iterations, ||b - D x||/||b||."""
+        bp = self.schur_prepare(b)
+        rhs = self.Ainv(bp, self.sites_odd)
+        bnorm = np.sqrt(self.redot(b, b, self.sites_all))
+        # ||b' - Mpc x|| = ||A rho|| <= (|alpha| + |beta|) ||rho||: stop on the bound
+        x_o, iters = self.cgls_op(self.Mpc_sym, self.Mpc_sym_dag, rhs, tol * bnorm / (abs(self.alpha) + abs(self.beta)), maxiter)
+        x = self.schur_reconstruct(b, x_o)
+        return x, iters, self.true_residual(b, x)
