@@ -122,19 +122,6 @@ int mdwf_half_decode(mdwf_ctx *ctx, const void *words_dev, const void *scales_de
  * (Mpc + Mpc^dagger applications in the last solve, all precisions), "sloppy_applications". */
 int mdwf_get_stat(const mdwf_ctx *ctx, const char *key, double *value);
 
-/* Measurement: run op (MDWF_OP_MPC or MDWF_OP_MPCDAG) `reps` times after `warmup`
- * untimed runs, in precision "fp64" | "fp32" | "half", on library-owned hash-filled vectors, timed with
- * CUDA events on the context's stream.  out4[0] = ms per application (both kernels), out4[1] / out4[2] =
- * ms per launch of its first / second kernel timed alone, out4[3] = kernels launched by this call.  For the 16-bit
- * Mpc the first kernel is the one mdwf_solve launches (K1 reading the B p stream of the fused CG update), unless the
- * option "bp_stream" is "0". */
-int mdwf_time_op(mdwf_ctx *ctx, int op, const char *precision, int reps, int warmup, double *out4);
-
-/* Measurement of the ALU roofline denominators: the device's fp32 fused-multiply-add
- * rate with scalar FFMA (tfma2[0]) and with the packed f32x2 FFMA2 the fp32-arithmetic kernels use (tfma2[1]),
- * in 1e12 FMA per second (two flops each), 16 independent chains per thread on every SM. */
-int mdwf_fma_rates(mdwf_ctx *ctx, double *tfma2);
-
 const char *mdwf_last_error(const mdwf_ctx *ctx);
 /* The fixed flop count per odd 5D site per Mpc application: 2880 + 48 L5. */
 int mdwf_flops_per_site(const mdwf_ctx *ctx);

@@ -16,7 +16,7 @@ OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG = 0, 1, 2, 3, 4
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
            "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
-           "mdwf_half_encode", "mdwf_half_decode"]
+           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates"]
 
 _lib = None
 
@@ -53,6 +53,7 @@ def lib():
         L.mdwf_flops_per_site.argtypes = [P]
         L.mdwf_time_op.argtypes = [P, I, ctypes.c_char_p, I, I, ctypes.POINTER(D)]
         L.mdwf_fma_rates.argtypes = [P, ctypes.POINTER(D)]
+        L.mdwf_l2_rates.argtypes = [P, ctypes.POINTER(D)]
         L.mdwf_half_encode.argtypes = [P, P, I, I, P, P]
         L.mdwf_half_decode.argtypes = [P, P, P, P, I]
         _lib = L
@@ -179,6 +180,12 @@ class Mdwf:
         out = (ctypes.c_double * 2)()
         _check(self.h, lib().mdwf_fma_rates(self.h, out))
         return out[0], out[1]
+
+    def l2_rates(self):
+        """GB/s: (LDG from L2, bulk copies from L2, LDG DRAM stream, bulk-copy DRAM stream) (mdwf_l2_rates)."""
+        out = (ctypes.c_double * 4)()
+        _check(self.h, lib().mdwf_l2_rates(self.h, out))
+        return tuple(out)
 
     def half_encode(self, x, via_fp64=False):
         """parity spinor [L5][Vh][4][3] -> (uint16 words [L5][Vh][24], fp32 scales [L5][Vh]) as the 16-bit format stores them"""

@@ -2,6 +2,7 @@
 // mixed-precision CG with reliable updates (S8-S10).  Host logic only; every arithmetic step runs in
 // the kernels of hop_kernels.cuh / blas_kernels.cu / layout_kernels.cu.
 #include "../../include/mdwf.h"
+#include "../../include/mdwf_bench.h"
 #include "mdwf_internal.h"
 
 #include <algorithm>
@@ -18,6 +19,7 @@ int mdwf_launch_hop_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop5_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_sdense_mma(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_S(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
@@ -25,6 +27,10 @@ int mdwf_launch_sdense_H(int, int, const SpinorBuf &, const SpinorBuf &, const v
 
 int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
 {
+    if (a.kver >= 5 && p == PREC_S) {        // v5 tile sweep; -1 = not covered, fall back to v3
+        const int rc = mdwf_launch_hop5_S(dag, pre, post, own, a, st);
+        if (rc != -1) return rc;
+    }
     if (a.kver >= 3 && p != PREC_D) {        // v3 family (fp32 arithmetic); -1 = not covered, fall back to v2
         const int rc = (p == PREC_S) ? mdwf_launch_hop3_S(dag, pre, post, own, a, st)
                                      : mdwf_launch_hop3_H(dag, pre, post, own, a, st);
@@ -469,8 +475,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
     } else if (k == "kernels") {
-        if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
-        else { c->err = "kernels must be v2|v3|v4"; return MDWF_EARG; }
+        if (v == "v5") c->kver = 5; else if (v == "v6") c->kver = 6; else if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
+        else { c->err = "kernels must be v2|v3|v4|v5"; return MDWF_EARG; }
     } else if (k == "bp_stream") {
         c->use_bp = atoi(value);
     } else if (k == "sweep_mb") {
@@ -824,59 +830,6 @@ int mdwf_blas_axpy(mdwf_ctx *c, double a, const void *x, void *y, long long n, i
     return MDWF_OK;
 }
 
-static int time_op_events(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4, cudaEvent_t e0, cudaEvent_t e1)
-{
-    TRY(check_ready(c));
-    if (!precision || !out4 || reps < 1 || warmup < 0 || (op != MDWF_OP_MPC && op != MDWF_OP_MPCDAG)) return MDWF_EARG;
-    const std::string pr(precision);
-    Prec p;
-    if (pr == "fp64") p = PREC_D; else if (pr == "fp32") p = PREC_S; else if (pr == "half") p = PREC_H;
-    else { c->err = "precision must be fp64|fp32|half"; return MDWF_EARG; }
-    SpinorBuf a, t, b;
-    TRY(get_spinor(c, "tm.a", p, &a));
-    TRY(get_spinor(c, "tm.t", p, &t));
-    TRY(get_spinor(c, "tm.b", p, &b));
-    CUDA_OK(c, mdwf_launch_fill(p, a, c->L5, c->Vh, 12345u, c->st));
-    CUDA_OK(c, mdwf_launch_fill(p, t, c->L5, c->Vh, 999u, c->st));
-    c->launches += 2;
-    const double l0 = c->launches;
-    for (int phase = 0; phase < 3; phase++) {     // 0: K1 + K2 back to back, 1: K1 alone, 2: K2 alone
-        for (int it = -warmup; it < reps; it++) {
-            if (it == 0) CUDA_OK(c, cudaEventRecord(e0, c->st));
-            // 16-bit Mpc: time the K1 the CG really launches (it reads the B p stream of the fused update)
-            const bool k1b = (op == MDWF_OP_MPC) && p == PREC_H && c->use_bp && bp_stream_available(c, p);
-            if (phase != 2) TRY(op == MDWF_OP_MPC ? (k1b ? op_Mpc_k1_from_B(c, p, a, t) : op_Mpc_k1(c, p, a, t)) : op_Mpcdag_k1(c, p, a, t));
-            if (phase != 1) TRY(op == MDWF_OP_MPC ? op_Mpc_k2(c, p, a, t, b) : op_Mpcdag_k2(c, p, a, t, b));
-        }
-        CUDA_OK(c, cudaEventRecord(e1, c->st));
-        CUDA_OK(c, cudaEventSynchronize(e1));
-        float ms = 0.f;
-        CUDA_OK(c, cudaEventElapsedTime(&ms, e0, e1));
-        out4[phase] = (double)ms / reps;
-    }
-    out4[3] = c->launches - l0;
-    return MDWF_OK;
-}
-int mdwf_time_op(mdwf_ctx *c, int op, const char *precision, int reps, int warmup, double *out4)
-{
-    cudaEvent_t e0, e1;
-    if (!c) return MDWF_EARG;
-    CUDA_OK(c, cudaEventCreate(&e0));
-    if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); c->err = "cudaEventCreate"; return MDWF_ECUDA; }
-    const int rc = time_op_events(c, op, precision, reps, warmup, out4, e0, e1);   // events are released on every path
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    return rc;
-}
-
-int mdwf_fma_rates(mdwf_ctx *c, double *tfma2)
-{
-    if (!c || !tfma2) return MDWF_EARG;
-    CUDA_OK(c, mdwf_measure_fma_rates(tfma2, c->st));
-    c->launches += 6;
-    return MDWF_OK;
-}
-
 int mdwf_get_stat(const mdwf_ctx *c, const char *key, double *value)
 {
     if (!c || !key || !value) return MDWF_EARG;
@@ -893,3 +846,6 @@ int mdwf_get_stat(const mdwf_ctx *c, const char *key, double *value)
 }
 
 }   // extern "C"
+
+// measurement entry points (include/mdwf_bench.h): not part of the solver boundary
+#include "mdwf_bench_api.inc"

@@ -76,13 +76,16 @@ struct HopArgs {
     double *partial;         // v3 kernels: if non-null, ||out||^2 partial sums, one per block (fused norm, S7)
     const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
     // POST = 1 in the v3 kernels (hop3_kernels.cuh): coef_hop * B A^{-1} as a blocked recurrence
-    int kver;                // host side: kernel family requested (2: hop_kernels.cuh, 3: hop3 all-LDG, 4: hop3 with TMA-staged z/t neighbours)
+    int kver;                // host side: kernel family requested (2: hop_kernels.cuh, 3: hop3 all-LDG, 4: hop3 with TMA-staged z/t neighbours, 5: hop5 tile sweep where covered)
     int r_ok;                // 1 when the recurrence form is usable (|kappa| < 1)
     float r_nk;              // -kappa = -beta/alpha
     float r_cpow;            // (-kappa)^S, S = slices per thread
     float r_bz, r_cz;        // coef_hop b5/alpha, coef_hop c5/alpha
     float r_qC[4];           // coef_hop (b5 p_j + c5 p_{j-1})/alpha, p_j = (-kappa)^{j+1}, p_{-1} = 1
     float r_qW[32];          // coef_hop * wall term of slice s (effective index): -g m_f (b5 (-kappa)^{s+1} + c5 (-kappa)^s)
+    // v5 tile-sweep kernels (hop5_kernels.cuh): tile geometry, filled by the launcher
+    int t5_NY, t5_nzq, t5_NT, t5_ntiles;   // 32-site groups along y, z-pairs per chunk, t-pairs, tiles
+    FastDiv t5_dNY, t5_dnzq, t5_dNT;
 };
 
 // hop family launcher.  dag: 0 H, 1 H^dagger.  pre: 0 none, 1 B on load.  post: 0 none, 1 dense

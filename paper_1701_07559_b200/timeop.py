@@ -22,6 +22,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--reconstruct", default=None)
     ap.add_argument("--fma-rates", action="store_true", help="also print the measured FFMA / FFMA2 rates")
+    ap.add_argument("--l2-rates", action="store_true", help="also print the measured L2 -> SM and DRAM streaming rates")
     ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value")
     args = ap.parse_args()
     build.build()
@@ -38,6 +39,9 @@ def main():
     if args.fma_rates:
         r = m.fma_rates()
         print(json.dumps({"ffma_tfma_per_s": r[0], "ffma2_tfma_per_s": r[1], "ffma_tflops": 2 * r[0], "ffma2_tflops": 2 * r[1]}), flush=True)
+    if args.l2_rates:
+        r = m.l2_rates()
+        print(json.dumps({"l2_ldg_GBs": r[0], "l2_bulk_GBs": r[1], "dram_ldg_GBs": r[2], "dram_bulk_GBs": r[3]}), flush=True)
     F = m.flops_per_site()
     for prec in args.prec.split(","):
         rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[prec]

@@ -1,4 +1,4 @@
-"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol include/mdwf.h declares,
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol include/*.h declares,
 validates arguments, and fails loudly (no fallback) when no CUDA device is present."""
 import os
 import re
@@ -16,7 +16,8 @@ def binding():
 
 
 def test_every_declared_symbol_is_exported(binding):
-    hdr = open(os.path.join(ROOT, "include", "mdwf.h")).read()
+    inc = os.path.join(ROOT, "include")
+    hdr = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     declared = set(re.findall(r"\b(mdwf_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(binding.EXPORTS), declared ^ set(binding.EXPORTS)
     lib = binding.lib()
