@@ -244,8 +244,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
         // 16-byte asynchronous copies (LDGSTS) spread over the lanes, completion signalled on the same mbarrier: bulk
         // copies of 256 B cost the TMA engine as much as whole groups (measured: 48 of them per slice double the kernel time).
         const unsigned char *gin = reinterpret_cast<const unsigned char *>(a.in);
-        const bool noy = a.kver == 6;     // TIMING EXPERIMENT ONLY (wrong results): skip the y-halo rows
-        const int nyu = noy ? 0 : (8 * NV * Lxh) / 32;                              // copies per lane per slice
+        const int nyu = (8 * NV * Lxh) / 32;                              // copies per lane per slice
         const int xoff = (lane & (Lxh - 1)) * SL::CH, rpw = 32 / Lxh, r0 = lane / Lxh;   // rows per warp instruction, this lane's row
         unsigned it = 0;
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -615,7 +614,8 @@ static inline bool hop5_geometry(HopArgs &a)
     // z-pairs per chunk: the input planes of a chunk's t-pair (4 t-planes with halo) should stay in L2 until the next t-pair
     int nzq = nzp;
     const long pair_bytes = (long)a.t5_NY * 2 * 2 * a.L5 * 3072 * 3;      // groups of one z-pair x t-pair, 3 streams, fp32
-    while (nzq > 1 && (nzq % 2 == 0) && nzq * pair_bytes > (48L << 20)) nzq /= 2;
+    const long budget = (a.t5_l2mb > 0 ? (long)a.t5_l2mb : 48L) << 20;
+    while (nzq > 1 && (nzq % 2 == 0) && nzq * pair_bytes > budget) nzq /= 2;
     a.t5_nzq = nzq;
     a.t5_NT = a.L[3] / 2;
     a.t5_ntiles = a.t5_NY * nzp * a.t5_NT;
@@ -654,6 +654,7 @@ template <class P>
 static int launch_hop5_prec(int dag, int pre, int post, int own, HopArgs a, cudaStream_t st)
 {
     if (!hop5_geometry(a)) return -1;
+    if (a.kver == 5 && a.t5_ntiles < 8 * 148) return -1;     // default (auto): a persistent CTA per SM needs several tiles per SM to pay; "kernels=v5" forces it
     if (!dag && pre == 0 && post == 0 && own == 2) return launch_hop5_l5<P, 0, 0, 0, 2>(a, st);   // K2
     if (!dag && pre == 0 && post == 1 && own == 0) return launch_hop5_l5<P, 0, 0, 1, 0>(a, st);   // K1 reading a precomputed B psi
     if (dag && pre == 0 && post == 1 && own == 0) return launch_hop5_l5<P, 1, 0, 1, 0>(a, st);    // K1^+

@@ -69,8 +69,10 @@ struct mdwf_ctx {
     double delta = 0.1;
     int max_update_interval = 0;
     int use_bp = 1;          // 16-bit Krylov vectors: let the CG update write B p for K1 (option "bp_stream")
-    int kver = 3;            // kernel family for fp32 arithmetic: 3 = hop3_kernels.cuh (link tile by TMA, spinors through registers),
+    int kver = 5;            // kernel family for fp32 arithmetic: 5 = hop5_kernels.cuh tile sweep where it applies, else as 3;
+                             // 3 = hop3_kernels.cuh (link tile by TMA, spinors through registers),
                              // 4 = the same with the t+- neighbour groups staged by TMA too, 2 = hop_kernels.cuh
+    int tile_l2_mb = 0;      // v5: L2 budget (MB) of the working set of a z-chunk of tiles; 0 = default 48
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
@@ -281,6 +283,7 @@ static void fill_recurrence(const mdwf_ctx *c, HopArgs &a)
 static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, HopArgs a)
 {
     a.kver = c->kver;
+    a.t5_l2mb = c->tile_l2_mb;
     if (post == 1 && p != PREC_D && a.kver >= 3) fill_recurrence(c, a);
     CUDA_OK(c, mdwf_launch_hop(p, dag, pre, post, own, a, c->st));
     c->launches += 1;
@@ -475,10 +478,12 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
     } else if (k == "kernels") {
-        if (v == "v5") c->kver = 5; else if (v == "v6") c->kver = 6; else if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
-        else { c->err = "kernels must be v2|v3|v4|v5"; return MDWF_EARG; }
+        if (v == "auto") c->kver = 5; else if (v == "v5") c->kver = 6; else if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
+        else { c->err = "kernels must be auto|v2|v3|v4|v5"; return MDWF_EARG; }
     } else if (k == "bp_stream") {
         c->use_bp = atoi(value);
+    } else if (k == "tile_l2_mb") {
+        c->tile_l2_mb = atoi(value);
     } else if (k == "sweep_mb") {
         c->sweep_mb = atoi(value);
     } else if (k == "stream") {

@@ -85,6 +85,7 @@ struct HopArgs {
     float r_qW[32];          // coef_hop * wall term of slice s (effective index): -g m_f (b5 (-kappa)^{s+1} + c5 (-kappa)^s)
     // v5 tile-sweep kernels (hop5_kernels.cuh): tile geometry, filled by the launcher
     int t5_NY, t5_nzq, t5_NT, t5_ntiles;   // 32-site groups along y, z-pairs per chunk, t-pairs, tiles
+    int t5_l2mb;                           // L2 budget (MB) of a z-chunk's working set; 0 = default 48
     FastDiv t5_dNY, t5_dnzq, t5_dNT;
 };
 
