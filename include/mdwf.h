@@ -54,7 +54,10 @@ enum { /* op codes of mdwf_apply */
     MDWF_OP_MPCDAG = 1,    /* Mpc^dagger : parity spinor -> parity spinor (S6)                   */
     MDWF_OP_MDAGM = 2,     /* Mpc^dagger Mpc                                                   */
     MDWF_OP_D = 3,         /* D          : full 5D spinor -> full 5D spinor                     */
-    MDWF_OP_DDAG = 4       /* D^dagger                                                          */
+    MDWF_OP_DDAG = 4,      /* D^dagger                                                          */
+    MDWF_OP_MPC_SYM = 5,   /* symmetric preconditioning:              */
+                           /*   Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B, parity spinor -> parity spinor */
+    MDWF_OP_MPCDAG_SYM = 6 /* Mpc_sym^dagger = 1 - (1/4) B^+ H'_oe A^{-+} B^+ H'_eo A^{-+}                      */
 };
 
 /* Create a context for an Lx x Ly x Lz x Lt x L5 lattice (all 4D extents even, 2 <= L5 <= 32) and the
@@ -84,7 +87,9 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *                     the next Mpc reads instead of applying B on load.
  *   "sweep_mb"        v2-v4: L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
  *   "max_update_interval"  force a reliable update at least every n iterations (default "0": only the delta rule).
- *   "matpc"           "asym" only (the operator Chroma uses).
+ *   "matpc"           "asym" (default; the operator Chroma uses) | "sym": Schur system mdwf_solve iterates on.
+ *                     sym: Mpc_sym x_o = A^{-1} b'_o with Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B ("significant reduction of
+ *                     the condition number"); same source preparation, reconstruction and returned residual.
  */
 int mdwf_set_option(mdwf_ctx *ctx, const char *key, const char *value);
 
@@ -92,7 +97,7 @@ int mdwf_set_option(mdwf_ctx *ctx, const char *key, const char *value);
 int mdwf_load_gauge(mdwf_ctx *ctx, const void *U_dev, int real_bytes);
 int mdwf_load_gauge_host(mdwf_ctx *ctx, const void *U_host, int real_bytes);
 
-/* out = op(in).  ops 0-2: parity spinors (odd sites); ops 3-4: full 5D spinors.  in_dev != out_dev. */
+/* out = op(in).  ops 0-2, 5, 6: parity spinors (odd sites); ops 3-4: full 5D spinors.  in_dev != out_dev. */
 int mdwf_apply(mdwf_ctx *ctx, int op, const void *in_dev, void *out_dev, int real_bytes);
 
 /* Solve D x = src on the full 5D lattice (fp64 buffers): Schur preparation b' = b_o - D_oe A^{-1} b_e,
@@ -111,6 +116,14 @@ int mdwf_solve_host(mdwf_ctx *ctx, const void *src_host, void *sol_host, double 
 int mdwf_blas_norm2(mdwf_ctx *ctx, const void *x_dev, long long n, int real_bytes, double *out);
 int mdwf_blas_redot(mdwf_ctx *ctx, const void *x_dev, const void *y_dev, long long n, int real_bytes, double *out);
 int mdwf_blas_axpy(mdwf_ctx *ctx, double a, const void *x_dev, void *y_dev, long long n, int real_bytes);
+
+/* 4D <-> 5D maps either side of the solve (Eq. (5), defines the quark field on the
+ * walls and the midpoint field of the residual-mass ratio).  4D fields are eta[t][z][y][x][spin][colour] (V4 x 24 reals).
+ * mdwf_wall_source: src(x,s) = delta_{s,0} P+ eta(x) + delta_{s,L5-1} P- eta(x) (lift = 0), or D_- applied to it (lift = 1;
+ * D_- = c5 D_W - 1 slice by slice, the source of the physical 4D propagator; needs the gauge field).
+ * mdwf_wall_project: q(x) = P- psi(x,0) + P+ psi(x,L5-1) (midpoint = 0) or Q(x) = P- psi(x,L5/2) + P+ psi(x,L5/2-1) (midpoint = 1). */
+int mdwf_wall_source(mdwf_ctx *ctx, const void *eta_dev, void *src_dev, int real_bytes, int lift);
+int mdwf_wall_project(mdwf_ctx *ctx, const void *psi_dev, void *q_dev, int real_bytes, int midpoint);
 
 /* The 16-bit storage format of the sloppy precision as it is stored (the paper
  * says only "double-half"): one fp32 scale m = max |component| per (site, s) and 24 unsigned 16-bit words

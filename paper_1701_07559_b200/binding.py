@@ -11,12 +11,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmdwf_b200.so")
 
 MDWF_OK, MDWF_EARG, MDWF_ENOGAUGE, MDWF_ECUDA, MDWF_ENOCONV, MDWF_ENOMEM = 0, -1, -2, -3, -4, -5
-OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG = 0, 1, 2, 3, 4
+OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG, OP_MPC_SYM, OP_MPCDAG_SYM = 0, 1, 2, 3, 4, 5, 6
 
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
            "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
-           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates"]
+           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project"]
 
 _lib = None
 
@@ -55,6 +55,8 @@ def lib():
         L.mdwf_fma_rates.argtypes = [P, ctypes.POINTER(D)]
         L.mdwf_l2_rates.argtypes = [P, ctypes.POINTER(D)]
         L.mdwf_half_encode.argtypes = [P, P, I, I, P, P]
+        L.mdwf_wall_source.argtypes = [P, P, P, I, I]
+        L.mdwf_wall_project.argtypes = [P, P, P, I, I]
         L.mdwf_half_decode.argtypes = [P, P, P, P, I]
         _lib = L
     return _lib
@@ -157,6 +159,22 @@ class Mdwf:
         assert x.is_cuda and x.is_contiguous()
         out = torch.empty_like(x)
         mdwf_apply(self.h, op, x.data_ptr(), out.data_ptr(), self._rb(x))
+        return out
+
+    def wall_source(self, eta, lift=False):
+        """4D field eta[t][z][y][x][4][3] -> 5D wall source (lift: with D_- applied)  (mdwf_wall_source)"""
+        import torch
+        assert eta.is_cuda and eta.is_contiguous()
+        out = torch.empty((self.L5,) + tuple(eta.shape), dtype=eta.dtype, device=eta.device)
+        _check(self.h, lib().mdwf_wall_source(self.h, eta.data_ptr(), out.data_ptr(), self._rb(eta), int(lift)))
+        return out
+
+    def wall_project(self, psi, midpoint=False):
+        """5D field -> q(x) on the walls (or the midpoint field)  (mdwf_wall_project)"""
+        import torch
+        assert psi.is_cuda and psi.is_contiguous()
+        out = torch.empty(tuple(psi.shape[1:]), dtype=psi.dtype, device=psi.device)
+        _check(self.h, lib().mdwf_wall_project(self.h, psi.data_ptr(), out.data_ptr(), self._rb(psi), int(midpoint)))
         return out
 
     def solve(self, src, tol=1e-10, maxiter=20000):

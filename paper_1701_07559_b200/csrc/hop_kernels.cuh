@@ -318,6 +318,8 @@ static int launch_hop_prec(int dag, int pre, int post, int own, const HopArgs &a
     if (!dag && pre == 1 && post == 0 && own == 1) return launch_hop_l5<P, 0, 1, 0, 1>(a, st);   // Schur prep/recon
     if (dag && pre == 0 && post == 1 && own == 0) return launch_hop_l5<P, 1, 0, 1, 0>(a, st);    // K1^+
     if (dag && pre == 0 && post == 2 && own == 3) return launch_hop_l5<P, 1, 0, 2, 3>(a, st);    // K2^+, D^+
+    if (!dag && pre == 0 && post == 1 && own == 1) return launch_hop_l5<P, 0, 0, 1, 1>(a, st);   // K2 of Mpc_sym: psi + coef A^{-1} H t
+    if (dag && pre == 0 && post == 2 && own == 1) return launch_hop_l5<P, 1, 0, 2, 1>(a, st);    // K2^+ of Mpc_sym^+: psi + coef B^+ H' u
     return (int)cudaErrorInvalidValue;
 }
 

@@ -268,3 +268,45 @@ int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed
     }
     return (int)cudaGetLastError();
 }
+
+// ---- 4D <-> 5D maps on canonical buffers (Eq. (5)) --------------------------
+// wall source: b(x,s) = delta_{s,0} P+ eta(x) + delta_{s,L5-1} P- eta(x); P+ keeps spins 0,1, P- spins 2,3 (gamma5 = diag(+,+,-,-))
+template <class T>
+__global__ void wall_inject_kernel(const T *eta, T *b, long V4, int L5)
+{
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;       // one complex number of the 4D field: (site, spin, colour)
+    if (i >= V4 * 12) return;
+    const int spin = (int)((i / 3) % 4);
+    const int s = (spin < 2) ? 0 : L5 - 1;
+    b[2 * ((long)s * V4 * 12 + i)] = eta[2 * i];
+    b[2 * ((long)s * V4 * 12 + i) + 1] = eta[2 * i + 1];
+}
+// q(x) = P- psi(x, sm) + P+ psi(x, sp): walls (sm = 0, sp = L5-1) or midpoint (sm = L5/2, sp = L5/2 - 1)
+template <class T>
+__global__ void wall_project_kernel(const T *psi, T *q, long V4, int sm, int sp)
+{
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= V4 * 12) return;
+    const int spin = (int)((i / 3) % 4);
+    const int s = (spin < 2) ? sp : sm;
+    q[2 * i] = psi[2 * ((long)s * V4 * 12 + i)];
+    q[2 * i + 1] = psi[2 * ((long)s * V4 * 12 + i) + 1];
+}
+int mdwf_launch_wall_inject(const void *eta, void *b, int real_bytes, long V4, int L5, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(b, 0, (size_t)L5 * V4 * 24 * real_bytes, st);
+    if (e != cudaSuccess) return (int)e;
+    const int T = 256;
+    const unsigned nb = (unsigned)((V4 * 12 + T - 1) / T);
+    if (real_bytes == 8) wall_inject_kernel<double><<<nb, T, 0, st>>>((const double *)eta, (double *)b, V4, L5);
+    else wall_inject_kernel<float><<<nb, T, 0, st>>>((const float *)eta, (float *)b, V4, L5);
+    return (int)cudaGetLastError();
+}
+int mdwf_launch_wall_project(const void *psi, void *q, int real_bytes, long V4, int sm, int sp, cudaStream_t st)
+{
+    const int T = 256;
+    const unsigned nb = (unsigned)((V4 * 12 + T - 1) / T);
+    if (real_bytes == 8) wall_project_kernel<double><<<nb, T, 0, st>>>((const double *)psi, (double *)q, V4, sm, sp);
+    else wall_project_kernel<float><<<nb, T, 0, st>>>((const float *)psi, (float *)q, V4, sm, sp);
+    return (int)cudaGetLastError();
+}

@@ -55,7 +55,7 @@ int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const Spinor
     }
 }
 
-enum { DENSE_BAINV = 0, DENSE_BAINV_DAG = 1, DENSE_AINV = 2, DENSE_KINDS = 3 };
+enum { DENSE_BAINV = 0, DENSE_BAINV_DAG = 1, DENSE_AINV = 2, DENSE_AINV_DAG = 3, DENSE_KINDS = 4 };
 
 struct mdwf_ctx {
     int L[4];
@@ -69,6 +69,7 @@ struct mdwf_ctx {
     double delta = 0.1;
     int max_update_interval = 0;
     int use_bp = 1;          // 16-bit Krylov vectors: let the CG update write B p for K1 (option "bp_stream")
+    int matpc_sym = 0;       // 0: asymmetric Schur operator (what Chroma uses), 1: symmetric (NEXT-1)
     int kver = 5;            // kernel family for fp32 arithmetic: 5 = hop5_kernels.cuh tile sweep where it applies, else as 3;
                              // 3 = hop3_kernels.cuh (link tile by TMA, spinors through registers),
                              // 4 = the same with the t+- neighbour groups staged by TMA too, 2 = hop_kernels.cuh
@@ -76,7 +77,7 @@ struct mdwf_ctx {
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
-    void *dense[2][DENSE_KINDS] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [0] double, [1] float
+    void *dense[2][DENSE_KINDS] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};   // [0] double, [1] float
     std::map<std::string, SpinorBuf> pool;
     std::map<std::string, void *> raw;
     double *partial = nullptr, *result_dev = nullptr, *result_host = nullptr;
@@ -153,6 +154,8 @@ static void build_tables(const mdwf_ctx *c, std::vector<double> out[DENSE_KINDS]
             out[DENSE_BAINV_DAG][n * n + j * n + i] = sm;
             out[DENSE_AINV][i * n + j] = Aip[i * n + j];
             out[DENSE_AINV][n * n + i * n + j] = Aim[i * n + j];
+            out[DENSE_AINV_DAG][j * n + i] = Aip[i * n + j];           // A^{-+} per chirality = transpose
+            out[DENSE_AINV_DAG][n * n + j * n + i] = Aim[i * n + j];
         }
 }
 
@@ -265,26 +268,26 @@ static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const Spinor
     return a;
 }
 // constants of the recurrence form of coef_hop * B A^{-1} (hop3_kernels.cuh)
-static void fill_recurrence(const mdwf_ctx *c, HopArgs &a)
+static void fill_recurrence(const mdwf_ctx *c, HopArgs &a, double b5, double c5)
 {
     const double ka = c->beta / c->alpha, nk = -ka, coef = a.coef_hop;
     const int S = mdwf_h3_slices(c->L5);
     a.r_ok = (std::fabs(ka) < 0.98) ? 1 : 0;
     a.r_nk = (float)nk;
     a.r_cpow = (float)std::pow(nk, S);
-    a.r_bz = (float)(coef * c->b5 / c->alpha);
-    a.r_cz = (float)(coef * c->c5 / c->alpha);
+    a.r_bz = (float)(coef * b5 / c->alpha);
+    a.r_cz = (float)(coef * c5 / c->alpha);
     for (int j = 0; j < 4; j++)
-        a.r_qC[j] = (float)(coef * (c->b5 * std::pow(nk, j + 1) + c->c5 * std::pow(nk, j)) / c->alpha);
+        a.r_qC[j] = (float)(coef * (b5 * std::pow(nk, j + 1) + c5 * std::pow(nk, j)) / c->alpha);
     const double g = 1.0 / (c->alpha * (1.0 + c->mf * std::pow(nk, c->L5)));
     for (int s = 0; s < 32; s++)
-        a.r_qW[s] = (s < c->L5) ? (float)(coef * (-g * c->mf) * (c->b5 * std::pow(nk, s + 1) + c->c5 * std::pow(nk, s))) : 0.f;
+        a.r_qW[s] = (s < c->L5) ? (float)(coef * (-g * c->mf) * (b5 * std::pow(nk, s + 1) + c5 * std::pow(nk, s))) : 0.f;
 }
-static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, HopArgs a)
+static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, HopArgs a, bool ainv_only = false)
 {
     a.kver = c->kver;
     a.t5_l2mb = c->tile_l2_mb;
-    if (post == 1 && p != PREC_D && a.kver >= 3) fill_recurrence(c, a);
+    if (post == 1 && p != PREC_D && a.kver >= 3) fill_recurrence(c, a, ainv_only ? 1.0 : c->b5, ainv_only ? 0.0 : c->c5);   // coef (B A^{-1}) or coef A^{-1}
     CUDA_OK(c, mdwf_launch_hop(p, dag, pre, post, own, a, c->st));
     c->launches += 1;
     return MDWF_OK;
@@ -367,6 +370,37 @@ static int op_Mpcdag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &
     if (p != PREC_D) c->sloppy_applications += 1;
     return MDWF_OK;
 }
+// ---- NEXT-1: symmetric preconditioning ----------------------------------------------
+// Mpc_sym in_o = in_o - (1/4) A^{-1} H_oe [B A^{-1} H_eo B in_o]: K1 as for Mpc, K2 with A^{-1} as its POST step and OWN = 1
+static int op_Ainv_dag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out);
+static int op_Mpc_sym(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out, double *norm2_out = nullptr)
+{
+    TRY(op_Mpc_k1(c, p, in, tmp));
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);
+    k2.coef_hop = -0.25; k2.dense = dense_ptr(c, p, DENSE_AINV);
+    const bool fused = norm2_out && fused_norm_available(c, p) && std::fabs(c->beta / c->alpha) < 0.98;
+    if (fused) { TRY(ensure_scalars(c)); k2.partial = c->hop_partial; }
+    TRY(run_hop(c, p, 0, 0, 1, 1, k2, true));
+    c->op_applications += 1;
+    if (p != PREC_D) c->sloppy_applications += 1;
+    return finish_norm(c, p, out, fused, norm2_out);
+}
+// Mpc_sym^+ in_o = in_o - (1/4) B^+ H'_oe [A^{-+} B^+ H'_eo (A^{-+} in_o)]: a site-local A^{-+} pass (w holds it), then K1^+ as for
+// Mpc^+ and K2^+ with OWN = 1
+static int op_Mpcdag_sym(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &w, const SpinorBuf &tmp, const SpinorBuf &out,
+                         double *norm2_out = nullptr)
+{
+    TRY(op_Ainv_dag(c, p, in, w));
+    TRY(op_Mpcdag_k1(c, p, w, tmp));
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);
+    k2.coef_hop = -0.25; k2.post_d = c->b5; k2.post_o = c->c5;
+    const bool fused = norm2_out && fused_norm_available(c, p);
+    if (fused) { TRY(ensure_scalars(c)); k2.partial = c->hop_partial; }
+    TRY(run_hop(c, p, 1, 0, 2, 1, k2));
+    c->op_applications += 1;
+    if (p != PREC_D) c->sloppy_applications += 1;
+    return finish_norm(c, p, out, fused, norm2_out);
+}
 // one parity of D: out_p = A in_p - (1/2) H_{p,pbar} B in_pbar
 static int op_D_parity(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_other, const SpinorBuf &in_same,
                        const SpinorBuf &out)
@@ -394,6 +428,13 @@ static int op_schur_hop(mdwf_ctx *c, Prec p, int parity, const SpinorBuf &in_oth
 static int op_Ainv(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out)
 {
     CUDA_OK(c, mdwf_launch_sdense(p, c->L5, c->Vh, in, out, dense_ptr(c, p, DENSE_AINV), c->st));
+    c->launches += 1;
+    return MDWF_OK;
+}
+
+static int op_Ainv_dag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out)
+{
+    CUDA_OK(c, mdwf_launch_sdense(p, c->L5, c->Vh, in, out, dense_ptr(c, p, DENSE_AINV_DAG), c->st));
     c->launches += 1;
     return MDWF_OK;
 }
@@ -489,7 +530,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "stream") {
         c->st = (cudaStream_t)(uintptr_t)strtoull(value, nullptr, 10);
     } else if (k == "matpc") {
-        if (v != "asym") { c->err = "only matpc=asym is implemented"; return MDWF_EARG; }
+        if (v == "asym") c->matpc_sym = 0; else if (v == "sym") c->matpc_sym = 1;
+        else { c->err = "matpc must be asym|sym"; return MDWF_EARG; }
     } else {
         c->err = "unknown option " + k;
         return MDWF_EARG;
@@ -553,7 +595,7 @@ int mdwf_load_gauge_host(mdwf_ctx *c, const void *U_host, int real_bytes)
 int mdwf_apply(mdwf_ctx *c, int op, const void *in_dev, void *out_dev, int real_bytes)
 {
     TRY(check_ready(c));
-    if (!in_dev || !out_dev || in_dev == out_dev || (real_bytes != 8 && real_bytes != 4) || op < 0 || op > 4) {
+    if (!in_dev || !out_dev || in_dev == out_dev || (real_bytes != 8 && real_bytes != 4) || op < 0 || op > MDWF_OP_MPCDAG_SYM) {
         c->err = "mdwf_apply: bad argument";
         return MDWF_EARG;
     }
@@ -562,10 +604,12 @@ int mdwf_apply(mdwf_ctx *c, int op, const void *in_dev, void *out_dev, int real_
     TRY(get_spinor(c, "ap.a", p, &a));
     TRY(get_spinor(c, "ap.b", p, &b));
     TRY(get_spinor(c, "ap.t", p, &t));
-    if (op <= MDWF_OP_MDAGM) {
+    if (op <= MDWF_OP_MDAGM || op == MDWF_OP_MPC_SYM || op == MDWF_OP_MPCDAG_SYM) {
         CUDA_OK(c, mdwf_launch_parity_in(p, in_dev, real_bytes, a, c->L5, c->Vh, c->st));
         if (op == MDWF_OP_MPC) TRY(op_Mpc(c, p, a, t, b));
         else if (op == MDWF_OP_MPCDAG) TRY(op_Mpcdag(c, p, a, t, b));
+        else if (op == MDWF_OP_MPC_SYM) TRY(op_Mpc_sym(c, p, a, t, b));
+        else if (op == MDWF_OP_MPCDAG_SYM) { TRY(get_spinor(c, "ap.u", p, &u)); TRY(op_Mpcdag_sym(c, p, a, u, t, b)); }
         else {
             TRY(get_spinor(c, "ap.u", p, &u));
             TRY(op_Mpc(c, p, a, t, u));
@@ -615,9 +659,18 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     TRY(get_spinor(c, "sv.ts", ps, &ts));
     TRY(get_spinor(c, "sv.xlo", pxl, &xlo));
     // 16-bit Krylov vectors: the CG update also writes B p, and p is double-buffered
-    const bool use_bp = (ps == PREC_H) && bp_stream_available(c, ps) && c->use_bp;
-    SpinorBuf p2, bpv;
+    const bool sym = c->matpc_sym != 0;                 // NEXT-1: iterate on Mpc_sym x_o = A^{-1} b'_o
+    const bool use_bp = (ps == PREC_H) && bp_stream_available(c, ps) && c->use_bp && !sym;
+    SpinorBuf p2, bpv, ws;
     if (use_bp) { TRY(get_spinor(c, "sv.p2", ps, &p2)); TRY(get_spinor(c, "sv.bp", ps, &bpv)); }
+    if (sym) TRY(get_spinor(c, "sv.ws", ps, &ws));      // A^{-+} r of Mpc_sym^+
+    // the Schur operator of the iteration and its adjoint in precision pr
+    auto opM = [&](Prec pr, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out, double *n2) -> int {
+        return sym ? op_Mpc_sym(c, pr, in, tmp, out, n2) : op_Mpc(c, pr, in, tmp, out, n2);
+    };
+    auto opMdag = [&](Prec pr, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out, double *n2) -> int {
+        return sym ? op_Mpcdag_sym(c, pr, in, ws, tmp, out, n2) : op_Mpcdag(c, pr, in, tmp, out, n2);
+    };
 
     c->iterations = 0; c->reliable_updates = 0; c->op_applications = 0; c->sloppy_applications = 0;
 
@@ -640,7 +693,13 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     TRY(op_Ainv(c, PDd, be, rhi));
     TRY(op_schur_hop(c, PDd, 1, rhi, bo, bp));
     // ||b - D x|| = ||b' - Mpc x_o|| once x_e is reconstructed, so the CG target is absolute: tol * ||b||
-    const double target = tol * bnorm;
+    double target = tol * bnorm;
+    if (sym) {
+        // right-hand side A^{-1} b'; the residual rho of the symmetric system gives b' - Mpc x_o = A rho, ||A rho|| <= (|alpha| + |beta|) ||rho||
+        TRY(op_Ainv(c, PDd, bp, te));
+        TRY(v_axpby(c, PDd, bp, 1.0, PDd, te, 0.0, PDd, nullptr, nullptr));
+        target /= (std::fabs(c->alpha) + std::fabs(c->beta));
+    }
 
     TRY(v_zero(c, PDd, xhi));
     TRY(v_zero(c, pxl, xlo));
@@ -651,7 +710,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     int k = 0, since_update = 0;
     if (!converged) {
         TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr)); // r_s = convert(r_hi)
-        TRY(op_Mpcdag(c, ps, rs, ts, g));                                   // g = Mpc^+ r
+        TRY(opMdag(ps, rs, ts, g, nullptr));                                // g = Mpc^+ r
         double gam = 0;
         SpinorBuf pc = p, pn = p2;                                          // current / next direction vector (use_bp)
         // fused update; with use_bp it also writes B p_new and flips the double buffer of p
@@ -666,7 +725,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
             return MDWF_OK;
         };
         auto apply_Mpc = [&](double *qq) -> int {                           // q = Mpc p, ||q||^2 from the K2 epilogue
-            if (!use_bp) return op_Mpc(c, ps, pc, ts, q, qq);
+            if (!use_bp) return opM(ps, pc, ts, q, qq);
             TRY(op_Mpc_k1_from_B(c, ps, bpv, ts));
             TRY(op_Mpc_k2(c, ps, pc, ts, q, qq));
             c->op_applications += 1;
@@ -696,7 +755,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
                 TRY(v_axpby(c, pxl, xlo, a, ps, pc, 1.0, pxl, &xlo, nullptr));  // x_lo += a p
                 TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
                 TRY(v_zero(c, pxl, xlo));
-                TRY(op_Mpc(c, PDd, xhi, te, rhi));
+                TRY(opM(PDd, xhi, te, rhi, nullptr));
                 TRY(v_axpby(c, PDd, rhi, 1.0, PDd, bp, -1.0, PDd, &rhi, &r2));   // r_hi = b' - Mpc x_hi
                 rn = std::sqrt(r2);
                 c->reliable_updates += 1;
@@ -704,10 +763,10 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
                 if (rn <= target) { converged = true; break; }
                 TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr));
                 rmax = rn;
-                TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));                 // g = Mpc^+ r, ||g||^2 fused
+                TRY(opMdag(ps, rs, ts, g, &gam_new));                       // g = Mpc^+ r, ||g||^2 fused
                 TRY(cg_update(0.0, gam_new / gam));                         // p = g + (gam'/gam) p   (x_lo is zero)
             } else {
-                TRY(op_Mpcdag(c, ps, rs, ts, g, &gam_new));
+                TRY(opMdag(ps, rs, ts, g, &gam_new));
                 TRY(cg_update(a, gam_new / gam));                           // x_lo += a p ; p = g + (gam'/gam) p
             }
             gam = gam_new;
@@ -776,6 +835,50 @@ int mdwf_solve_host(mdwf_ctx *c, const void *src_host, void *sol_host, double to
     CUDA_OK(c, cudaMemcpyAsync(sol_host, sol, bytes, cudaMemcpyDeviceToHost, c->st));
     CUDA_OK(c, cudaStreamSynchronize(c->st));
     return rc;
+}
+
+// ---- NEXT-3: 4D <-> 5D maps (Eq. (5)) ------------------------------------------------------------------
+int mdwf_wall_source(mdwf_ctx *c, const void *eta_dev, void *src_dev, int real_bytes, int lift)
+{
+    if (!c || !eta_dev || !src_dev || eta_dev == src_dev || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    const long V4 = 2L * c->Vh;
+    if (!lift) {
+        CUDA_OK(c, mdwf_launch_wall_inject(eta_dev, src_dev, real_bytes, V4, c->L5, c->st));
+        c->launches += 1;
+        CUDA_OK(c, cudaStreamSynchronize(c->st));
+        return MDWF_OK;
+    }
+    // D_- b = (c5 D_W - 1) b = beta b - (c5/2) H b, slice by slice, in fp64: per parity one hop launch with the own-site term beta b
+    TRY(check_ready(c));
+    void *w = nullptr;
+    TRY(get_raw(c, "map.w", (size_t)c->L5 * V4 * 24 * real_bytes, &w));
+    CUDA_OK(c, mdwf_launch_wall_inject(eta_dev, w, real_bytes, V4, c->L5, c->st));
+    SpinorBuf e, o, te, to;
+    TRY(get_spinor(c, "ap.a", PREC_D, &e));
+    TRY(get_spinor(c, "ap.b", PREC_D, &o));
+    TRY(get_spinor(c, "ap.t", PREC_D, &te));
+    TRY(get_spinor(c, "ap.u", PREC_D, &to));
+    CUDA_OK(c, mdwf_launch_full_in(PREC_D, w, real_bytes, e, c->L, c->L5, 0, c->st));
+    CUDA_OK(c, mdwf_launch_full_in(PREC_D, w, real_bytes, o, c->L, c->L5, 1, c->st));
+    for (int parity = 0; parity < 2; parity++) {
+        HopArgs a = base_args(c, PREC_D, parity, parity ? e : o, parity ? &o : &e, parity ? to : te);
+        a.coef_hop = -0.5 * c->c5; a.own_d = c->beta; a.own_o = 0.0;
+        TRY(run_hop(c, PREC_D, 0, 0, 0, 2, a));
+    }
+    CUDA_OK(c, mdwf_launch_full_out(PREC_D, te, src_dev, real_bytes, c->L, c->L5, 0, c->st));
+    CUDA_OK(c, mdwf_launch_full_out(PREC_D, to, src_dev, real_bytes, c->L, c->L5, 1, c->st));
+    c->launches += 5;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
+}
+int mdwf_wall_project(mdwf_ctx *c, const void *psi_dev, void *q_dev, int real_bytes, int midpoint)
+{
+    if (!c || !psi_dev || !q_dev || psi_dev == q_dev || (real_bytes != 8 && real_bytes != 4)) return MDWF_EARG;
+    const int sm = midpoint ? c->L5 / 2 : 0, sp = midpoint ? c->L5 / 2 - 1 : c->L5 - 1;
+    CUDA_OK(c, mdwf_launch_wall_project(psi_dev, q_dev, real_bytes, 2L * c->Vh, sm, sp, c->st));
+    c->launches += 1;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
 }
 
 // ---- the 16-bit storage format, as stored (bit-exact tests of the quantiser) ------------------------------------------

@@ -139,6 +139,10 @@ int mdwf_launch_gauge_in(Prec p, const void *canon, int real_bytes, void *dst, c
 int mdwf_launch_half_export(const SpinorBuf &src, void *words, void *scales, int L5, int Vh, cudaStream_t st);
 int mdwf_launch_half_import(const void *words, const void *scales, const SpinorBuf &dst, int L5, int Vh, cudaStream_t st);
 
+// 4D <-> 5D maps on canonical buffers (NEXT-3): wall source injection, wall / midpoint projection
+int mdwf_launch_wall_inject(const void *eta, void *b, int real_bytes, long V4, int L5, cudaStream_t st);
+int mdwf_launch_wall_project(const void *psi, void *q, int real_bytes, long V4, int sm, int sp, cudaStream_t st);
+
 // deterministic pseudo-random fill in [-1,1] (timing inputs only)
 int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st);
 

@@ -33,9 +33,9 @@ def test_create_validates_arguments(binding):
     h = binding.mdwf_create(4, 4, 4, 4, 12, 1.1, 1.5, 0.5, 0.005)
     assert binding.mdwf_flops_per_site(h) == 2880 + 48 * 12
     for k, v in (("ladder", "dsh"), ("reconstruct", "12"), ("apply_precision", "half"), ("reliable_delta", "0.2"),
-                 ("matpc", "asym")):
+                 ("matpc", "asym"), ("matpc", "sym"), ("kernels", "auto"), ("kernels", "v5"), ("tile_l2_mb", "64")):
         binding.mdwf_set_option(h, k, v)
-    for k, v in (("ladder", "x"), ("reconstruct", "8"), ("matpc", "sym"), ("nope", "1"), ("reliable_delta", "2")):
+    for k, v in (("ladder", "x"), ("reconstruct", "8"), ("matpc", "both"), ("kernels", "v9"), ("nope", "1"), ("reliable_delta", "2")):
         with pytest.raises(binding.MdwfError):
             binding.mdwf_set_option(h, k, v)
     binding.mdwf_destroy(h)
