@@ -136,9 +136,11 @@ def run_reference(args, rank, world):
 
 def workload_config(cfg, args):
     return {"workload": "BASELINE.json configs[%d]: %s, M5=%g b5=%g c5=%g m_f=%g, links exp(i %g H) seed %d, "
-                        "Gaussian source, ladder %s, reconstruct %d, tol 1e-10"
+                        "%s, ladder %s, reconstruct %d, tol 1e-10%s"
                         % (args.workload, cfg["name"], cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], cfg["eps"],
-                           cfg["seed"], cfg["ladder"], cfg["reconstruct"]),
+                           cfg["seed"], "point source at the origin x 12 spin-colour columns per step" if cfg["source"] == "point12"
+                           else "Gaussian source", cfg["ladder"], cfg["reconstruct"],
+                           "".join(", " + kv for kv in getattr(args, "opt", []))),
             "parallelism": "replicas only: one right-hand side per GPU, no data-path collective",
             "l2": "every vector of the step (>= 0.9 GB) is larger than the 126 MB L2; no explicit flush"}
 
@@ -153,6 +155,10 @@ def main():
     ap.add_argument("--ref-tslices", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--op-reps", type=int, default=20)
+    ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value (e.g. matpc=sym, kernels=v3)")
+    ap.add_argument("--oracle-solve", action="store_true",
+                    help="also run the FULL oracle CG solve of this workload on the host cores and report its iterations and seconds "
+                         "beside the GPU's (feasible for workloads 0 and 1)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -186,22 +192,32 @@ def main():
 
     # ---- inputs: same gauge field on every rank, one right-hand side per rank ---------------------------
     U = inputs.gauge_field(L, cfg["eps"], cfg["seed"], device="cuda")
-    src = inputs.gaussian_source(L, L5, replicas.source_seed(cfg["seed"], rank), device="cuda")
+    if cfg["source"] == "point12":      # configs[2]: the 12 spin-colour columns of a point source at the origin; a step solves all of them
+        srcs = [inputs.point_source(L, L5, sp, col, device="cuda") for sp in range(4) for col in range(3)]
+    else:
+        srcs = [inputs.gaussian_source(L, L5, replicas.source_seed(cfg["seed"], rank), device="cuda")]
+    src = srcs[0]
     m = binding.Mdwf(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"])
     m.set_option("reconstruct", cfg["reconstruct"])
     m.set_option("ladder", cfg["ladder"])
+    for kv in args.opt:
+        m.set_option(*kv.split("=", 1))
     m.load_gauge(U)
     F = m.flops_per_site()
     sol = torch.empty_like(src)
     tol, maxiter = 1e-10, 100000
 
-    def one_solve(host=False, s=None, x=None):
-        s = src if s is None else s
+    def one_solve(host=False, ss=None, x=None):
+        """one step: every right-hand side of the workload (1, or the 12 columns of configs[2])"""
+        ss = srcs if ss is None else ss
         x = sol if x is None else x
-        rc, it, tr = binding.mdwf_solve(m.h, s.data_ptr(), x.data_ptr(), tol, maxiter, host=host)
-        if rc != 0 or not (tr <= tol * 1.001):
-            raise SystemExit("solve failed: rc=%d true residual %.3e" % (rc, tr))
-        return it, tr, m.stat("op_applications"), m.stat("solve_seconds")
+        its, trs, na, sec = [], [], 0.0, 0.0
+        for s in ss:
+            rc, it, tr = binding.mdwf_solve(m.h, s.data_ptr(), x.data_ptr(), tol, maxiter, host=host)
+            if rc != 0 or not (tr <= tol * 1.001):
+                raise SystemExit("solve failed: rc=%d true residual %.3e" % (rc, tr))
+            its.append(it); trs.append(tr); na += m.stat("op_applications"); sec += m.stat("solve_seconds")
+        return max(its), max(trs), na, sec
 
     # ---- device-resident steps -----------------------------------------------------------------------------
     for _ in range(args.warmup):
@@ -226,19 +242,20 @@ def main():
     iters, true_res, n_upd = it, tr, m.stat("reliable_updates")
 
     # ---- end to end: host buffers, H2D of the source and D2H of the solution inside the timed region ----------
-    src_h = src.cpu().pin_memory()
+    srcs_h = [x.cpu().pin_memory() for x in srcs]
+    src_h = srcs_h[0]
     sol_h = torch.empty_like(src_h).pin_memory()
-    one_solve(True, src_h, sol_h)
+    one_solve(True, srcs_h, sol_h)
     barrier()
     t0 = time.perf_counter()
     apps_e = 0
     for _ in range(args.steps):
-        apps_e += one_solve(True, src_h, sol_h)[2]
+        apps_e += one_solve(True, srcs_h, sol_h)[2]
     barrier()
     e2e_s = time.perf_counter() - t0
     apps_e_all, e2e_s_max = replicas.aggregate(apps_e, e2e_s, device="cuda")
     e2e_value = apps_e_all * F * h / e2e_s_max / 1e12
-    nbytes = src_h.numel() * 16
+    nbytes = src_h.numel() * 16 * len(srcs)
 
     # ---- per-kernel Dslash numbers and the roofline of the dominant kernel -------------------------------------
     gl = {18: {"fp64": 8, "fp32": 4, "half": 2}, 12: {"fp64": 8, "fp32": 4, "half": 2}}
@@ -262,6 +279,8 @@ def main():
     b1 = (2 * (24 * rb + extra) + 8 * recon * rb / L5) * h      # K1 / K1+: read one vector, write one, 8 links / L5
     b2 = (3 * (24 * rb + extra) + 8 * recon * rb / L5) * h      # K2 / K2+: read two vectors, write one
     fam = "hop_kernel" if sloppy == "fp64" else "hop3_kernel"
+    tiles = (L[1] * (L[0] // 2) // 32) * (L[2] // 2) * (L[3] // 2) if (L[0] // 2) in (2, 4, 8, 16) and (L[1] * (L[0] // 2)) % 32 == 0 else 0
+    fam5 = "hop5_kernel" if (sloppy == "fp32" and L5 in (8, 12) and tiles >= 8 * 148) else fam   # tile-sweep kernels (not for K1 with B on load)
     pname = {"fp64": "PD", "fp32": "PS", "half": "PH"}[sloppy]
     k1b = sloppy == "half"                                      # 16-bit CG: K1 reads the B p stream, no B on load
     mp, md = mpc["Mpc_%s" % sloppy], mpc["Mpcdag_%s" % sloppy]
@@ -269,10 +288,10 @@ def main():
         ("%s<%s,0,%d,1,0,%d,3> (K1 of Mpc: t_e = B A^-1 H_eo %s)" % (fam, pname, 0 if k1b else 1, L5,
                                                                   "(B psi)_o, B psi streamed by the CG update" if k1b else "B psi_o"),
          mp["ms_k1"], b1, 1320 + (0 if k1b else 72) + 72 + 48 * L5 - 24, "k1"),
-        ("%s<%s,0,0,0,2,%d,3> (K2 of Mpc: A psi_o - 1/4 H_oe t_e)" % (fam, pname, L5), mp["ms_k2"], b2, 1320 + 72 + 48, "k2"),
-        ("%s<%s,1,0,1,0,%d,3> (K1 of Mpc^dagger: u_e = A^-+ B^+ H'_eo psi_o)" % (fam, pname, L5), md["ms_k1"], b1,
+        ("%s<%s,0,0,0,2,%d> (K2 of Mpc: A psi_o - 1/4 H_oe t_e)" % (fam5, pname, L5), mp["ms_k2"], b2, 1320 + 72 + 48, "k2"),
+        ("%s<%s,1,0,1,0,%d> (K1 of Mpc^dagger: u_e = A^-+ B^+ H'_eo psi_o)" % (fam5, pname, L5), md["ms_k1"], b1,
          1320 + 72 + 48 * L5 - 24, "k1"),
-        ("%s<%s,1,0,2,3,%d,3> (K2 of Mpc^dagger: A^+ psi_o - 1/4 B^+ H'_oe u_e)" % (fam, pname, L5), md["ms_k2"], b2,
+        ("%s<%s,1,0,2,3,%d> (K2 of Mpc^dagger: A^+ psi_o - 1/4 B^+ H'_oe u_e)" % (fam5, pname, L5), md["ms_k2"], b2,
          1320 + 72 + 72 + 48, "k2"),
     ]
     kname, k_ms, k_bytes, k_flops_site, k_key = max(cands, key=lambda c: c[1])
@@ -282,7 +301,7 @@ def main():
                 "algorithmic_bytes_per_launch": k_bytes, "ms_per_launch": k_ms,
                 "all_hop_kernels_ms": {c[0].split(" ")[0]: c[1] for c in cands}}
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
-    tf = os.path.join(ROOT, "profiles", "r01_traffic.csv")   # dram bytes per launch from the committed ncu capture
+    tf = os.path.join(ROOT, "profiles", "r02_traffic.csv")   # dram bytes per launch from the committed ncu capture
     if os.path.exists(tf):
         for ln in open(tf).read().splitlines()[1:]:
             k, _, v = ln.partition(",")
@@ -319,6 +338,20 @@ def main():
         nts = min(L[3], args.ref_tslices)
         r = oracle_sample(cfg, U.cpu().numpy(), src_h.numpy(), nts)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        # the oracle's time for the operator work of one CG iteration on the whole lattice, EXTRAPOLATED from the sample,
+        # and for the whole solve at the GPU's iteration count (BLAS-1 not included): context, labelled as extrapolated
+        per_it = r["seconds_per_pass"] * L[3] / nts
+        line["cpu_baseline"]["extrapolated"] = {
+            "oracle_seconds_per_cg_iteration": per_it,
+            "oracle_solve_seconds_at_gpu_iterations": per_it * int(iters) * len(srcs),
+            "note": "sample seconds x (Lt / sampled time slices) x GPU iteration count x right-hand sides; not measured"}
+        if args.oracle_solve:
+            from oracle import mdwf_oracle as mo
+            orc = mo.MdwfOracle(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], U.cpu().numpy())
+            t0 = time.perf_counter()
+            x_ref, it_ref, res_ref = orc.solve(src_h.numpy(), tol=1e-10)
+            line["cpu_baseline"]["oracle_full_solve"] = {"iterations": int(it_ref), "seconds": time.perf_counter() - t0,
+                                                         "true_residual": res_ref, "gpu_iterations": int(iters)}
     if rank == 0:
         print(json.dumps(line), flush=True)
     m.close()

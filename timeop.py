@@ -1,6 +1,6 @@
 """Time (or profile under ncu) the fused Mpc / Mpc^dagger kernels on one of BASELINE.json's workloads.
 
-  python -m paper_1701_07559_b200.timeop --workload 3 --prec fp32,half --reps 5 --warmup 2
+  python timeop.py --workload 3 --prec fp32,half --reps 5 --warmup 2
 
 Prints one JSON line per (op, precision): ms per application and per kernel, model GB/s, TFLOP/s.
 Few launches, so it is the command the ncu captures under profiles/ are taken with.
@@ -10,7 +10,7 @@ import json
 
 import torch
 
-from . import binding, build, inputs
+from paper_1701_07559_b200 import binding, build, inputs
 
 
 def main():
