@@ -125,6 +125,15 @@ int mdwf_blas_axpy(mdwf_ctx *ctx, double a, const void *x_dev, void *y_dev, long
 int mdwf_wall_source(mdwf_ctx *ctx, const void *eta_dev, void *src_dev, int real_bytes, int lift);
 int mdwf_wall_project(mdwf_ctx *ctx, const void *psi_dev, void *q_dev, int real_bytes, int midpoint);
 
+/* Gradient-flow smearing of the gauge field (Sec. III: "an infinitesimal stout-smearing
+ * procedure", t_gf = 1.0; App. D: "the Symanzik action ... step size eps = 0.03").  U_dev: canonical gauge field in
+ * fp64, flowed IN PLACE by nsteps steps of Luescher's third-order Runge-Kutta of size eps (flow time nsteps * eps) under
+ * dV/dt = -g0^2 {dS/dV} V; action 0 = Wilson flow (plaquette), 1 = tree-level Symanzik (c0 = 5/3, c1 = -1/12); periodic
+ * boundaries.  The flowed field is what mdwf_load_gauge should then be given.  plaq_out (may be null) receives the mean
+ * plaquette <Re tr P>/3 of the flowed field; mdwf_plaquette returns it for any field (deterministic reduction). */
+int mdwf_gradient_flow(mdwf_ctx *ctx, void *U_dev, double eps, int nsteps, int action, double *plaq_out);
+int mdwf_plaquette(mdwf_ctx *ctx, const void *U_dev, double *out);
+
 /* The 16-bit storage format of the sloppy precision as it is stored (the paper
  * says only "double-half"): one fp32 scale m = max |component| per (site, s) and 24 unsigned 16-bit words
  * u = round_to_nearest_even(v * (32767 / m)) + 32768, decoded as (u - 32768) * (m * (1 / 32767)) in fp32.

@@ -16,7 +16,7 @@ OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG, OP_MPC_SYM, OP_MPCDAG_SYM = 0, 1, 2,
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
            "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
-           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project"]
+           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project", "mdwf_gradient_flow", "mdwf_plaquette"]
 
 _lib = None
 
@@ -56,6 +56,8 @@ def lib():
         L.mdwf_l2_rates.argtypes = [P, ctypes.POINTER(D)]
         L.mdwf_half_encode.argtypes = [P, P, I, I, P, P]
         L.mdwf_wall_source.argtypes = [P, P, P, I, I]
+        L.mdwf_gradient_flow.argtypes = [P, P, D, I, I, ctypes.POINTER(D)]
+        L.mdwf_plaquette.argtypes = [P, P, ctypes.POINTER(D)]
         L.mdwf_wall_project.argtypes = [P, P, P, I, I]
         L.mdwf_half_decode.argtypes = [P, P, P, P, I]
         _lib = L
@@ -160,6 +162,22 @@ class Mdwf:
         out = torch.empty_like(x)
         mdwf_apply(self.h, op, x.data_ptr(), out.data_ptr(), self._rb(x))
         return out
+
+    def gradient_flow(self, U, eps, nsteps, action="wilson"):
+        """flow the canonical fp64 gauge field U in place; returns the mean plaquette of the flowed field  (mdwf_gradient_flow)"""
+        import torch
+        assert U.is_cuda and U.is_contiguous() and U.dtype == torch.complex128
+        out = ctypes.c_double()
+        _check(self.h, lib().mdwf_gradient_flow(self.h, U.data_ptr(), float(eps), int(nsteps), {"wilson": 0, "symanzik": 1}[action],
+                                                ctypes.byref(out)))
+        return out.value
+
+    def plaquette(self, U):
+        import torch
+        assert U.is_cuda and U.is_contiguous() and U.dtype == torch.complex128
+        out = ctypes.c_double()
+        _check(self.h, lib().mdwf_plaquette(self.h, U.data_ptr(), ctypes.byref(out)))
+        return out.value
 
     def wall_source(self, eta, lift=False):
         """4D field eta[t][z][y][x][4][3] -> 5D wall source (lift: with D_- applied)  (mdwf_wall_source)"""

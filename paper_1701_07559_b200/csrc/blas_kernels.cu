@@ -86,12 +86,30 @@ template <> struct CompT<PS, PH, PD> { using T = double; };
 template <> struct CompT<PH, PS, PD> { using T = double; };
 template <> struct CompT<PH, PH, PD> { using T = double; };
 
+// CG scalars kept on the device: while a coefficient pointer is set, the (a, b) of mdwf_launch_axpby / xpupdate / xpupdate_b
+// are multiplied by coef[0], coef[1] read in the kernel, so that alpha = gamma / ||q||^2 and beta = gamma' / gamma never
+// travel to the host ("unless kept on device")
+static thread_local const double *tl_coef = nullptr;
+void mdwf_blas_set_coef(const double *coef_dev) { tl_coef = coef_dev; }
+// S: [1] gamma, [2] ||q||^2, [3] ||r||^2, [4] gamma', [5..6] (alpha, 1) for r -= alpha q, [7..8] (alpha, beta) for the x / p update
+__global__ void cg_scalars_kernel(double *S, int mode)
+{
+    if (mode == 0) { const double al = S[1] / S[2]; S[5] = al; S[6] = 1.0; S[7] = al; }
+    else { S[8] = S[4] / S[1]; S[1] = S[4]; }
+}
+int mdwf_launch_cg_scalars(double *S, int mode, cudaStream_t st)
+{
+    cg_scalars_kernel<<<1, 1, 0, st>>>(S, mode);
+    return (int)cudaGetLastError();
+}
+
 template <class PO, class PX, class PY, bool HASY, bool NORM>
 __global__ void __launch_bounds__(RED_THREADS)
 axpby_kernel(void *out, float *out_norm, double a, const void *x, const float *xn, double b, const void *y,
-             const float *yn, int L5, long Vh, double *partial)
+             const float *yn, int L5, long Vh, double *partial, const double *coef)
 {
     using RO = typename PO::R;
+    if (coef) { a *= coef[0]; b *= coef[1]; }        // CG scalars kept on the device (mdwf_blas_set_coef)
     // grid = (blocks over the sites of one s-slice, L5): no integer division in the loop
     const int s = blockIdx.y;
     double sum = 0.0;
@@ -154,7 +172,7 @@ static int axpby_xy(const SpinorBuf &out, double a, const SpinorBuf &x, double b
     const dim3 nb = site_grid(L5, Vh);
     const bool hasy = (y.v != nullptr);
     const bool norm = (partial != nullptr);
-#define AX(HY, NM) axpby_kernel<PO, PX, PY, HY, NM><<<nb, RED_THREADS, 0, st>>>(out.v, out.norm, a, x.v, x.norm, b, y.v, y.norm, L5, Vh, partial)
+#define AX(HY, NM) axpby_kernel<PO, PX, PY, HY, NM><<<nb, RED_THREADS, 0, st>>>(out.v, out.norm, a, x.v, x.norm, b, y.v, y.norm, L5, Vh, partial, tl_coef)
     if (hasy && norm) AX(true, true);
     else if (hasy) AX(true, false);
     else if (norm) AX(false, true);
@@ -230,8 +248,10 @@ int mdwf_launch_reduce(int kind, Prec px, const SpinorBuf &x, Prec py, const Spi
 // ---- fused CG update: x += a p ; p = g + b p  (one read of p instead of two) --------------------------
 template <class PX, class PP>
 __global__ void __launch_bounds__(RED_THREADS)
-xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, const void *g, const float *gn, int L5, long Vh)
+xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, const void *g, const float *gn, int L5, long Vh,
+                const double *coef)
 {
+    if (coef) { a *= coef[0]; b *= coef[1]; }
     const int s = blockIdx.y;
     for (long cb = (long)blockIdx.x * RED_THREADS + threadIdx.x; cb < Vh; cb += (long)gridDim.x * RED_THREADS) {
         typename PP::R vp[24], vg[24];
@@ -257,8 +277,9 @@ xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, cons
 template <class PX, class PP>
 __global__ void __launch_bounds__(128)
 xpupdate_b_kernel(void *x, float *xn, double a, const void *p, const float *pn, double b, const void *g, const float *gn,
-                  void *pnew, float *pnewn, void *bp, float *bpn, float b5, float c5, float mf, int L5, long Vh)
+                  void *pnew, float *pnewn, void *bp, float *bpn, float b5, float c5, float mf, int L5, long Vh, const double *coef)
 {
+    if (coef) { a *= coef[0]; b *= coef[1]; }
     // one thread walks the L5 slices of one 4D site, so every slice of p and g is loaded once: the new p of slice
     // s+1 is formed one step ahead, its lower spins feed B at s and its upper spins feed B at s+2
     using T = typename CompT<PX, PP, PP>::T;
@@ -313,7 +334,7 @@ int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBu
 {
     const int nb = (Vh + 127) / 128;
 #define XB(PX) xpupdate_b_kernel<PX, PH><<<nb, 128, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, pnew.v, \
-                                                                     pnew.norm, bp.v, bp.norm, (float)b5, (float)c5, (float)mf, L5, Vh)
+                                                                     pnew.norm, bp.v, bp.norm, (float)b5, (float)c5, (float)mf, L5, Vh, tl_coef)
     if (px == PREC_S) XB(PS);
     else if (px == PREC_H) XB(PH);
     else return (int)cudaErrorInvalidValue;
@@ -326,7 +347,7 @@ static int xpupdate_p(Prec pp, const SpinorBuf &x, double a, const SpinorBuf &p,
                       cudaStream_t st)
 {
     const dim3 nb = site_grid(L5, Vh);
-#define XP(PP) xpupdate_kernel<PX, PP><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, L5, Vh)
+#define XP(PP) xpupdate_kernel<PX, PP><<<nb, RED_THREADS, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, L5, Vh, tl_coef)
     switch (pp) {
     case PREC_D: XP(PD); break;
     case PREC_S: XP(PS); break;

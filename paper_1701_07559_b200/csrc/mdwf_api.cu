@@ -81,6 +81,7 @@ struct mdwf_ctx {
     std::map<std::string, SpinorBuf> pool;
     std::map<std::string, void *> raw;
     double *partial = nullptr, *result_dev = nullptr, *result_host = nullptr;
+    int defer_slot = -1;             // >= 0: reductions leave their result in result_dev[defer_slot] and are NOT read back
     double *hop_partial = nullptr;   // one ||out||^2 partial per block of a hop launch (fused norms)
     // stats
     double launches = 0, iterations = 0, reliable_updates = 0, solve_seconds = 0, true_residual = 0;
@@ -194,7 +195,7 @@ static int ensure_scalars(mdwf_ctx *c)
 {
     if (c->partial) return MDWF_OK;
     CUDA_OK(c, cudaMalloc((void **)&c->partial, sizeof(double) * mdwf_reduce_max_blocks()));
-    CUDA_OK(c, cudaMalloc((void **)&c->result_dev, sizeof(double) * 4));
+    CUDA_OK(c, cudaMalloc((void **)&c->result_dev, sizeof(double) * 16));
     CUDA_OK(c, cudaMalloc((void **)&c->hop_partial, sizeof(double) * (size_t)((c->Vh + 31) / 32)));
     CUDA_OK(c, cudaMallocHost((void **)&c->result_host, sizeof(double) * 4));
     return MDWF_OK;
@@ -213,18 +214,20 @@ static int v_axpby(mdwf_ctx *c, Prec po, const SpinorBuf &out, double a, Prec px
 {
     SpinorBuf none;
     TRY(ensure_scalars(c));
+    const bool defer = c->defer_slot >= 0;
     CUDA_OK(c, mdwf_launch_axpby(po, out, a, px, x, b, py, y ? *y : none, c->L5, c->Vh, norm2_out ? c->partial : nullptr,
-                                 c->result_dev, c->st));
+                                 c->result_dev + (defer ? c->defer_slot : 0), c->st));
     c->launches += norm2_out ? 2 : 1;
-    if (norm2_out) TRY(fetch_scalar(c, norm2_out));
+    if (norm2_out && !defer) TRY(fetch_scalar(c, norm2_out));
     return MDWF_OK;
 }
 static int v_norm2(mdwf_ctx *c, Prec p, const SpinorBuf &x, double *out)
 {
     TRY(ensure_scalars(c));
-    CUDA_OK(c, mdwf_launch_reduce(0, p, x, p, x, c->L5, c->Vh, c->partial, c->result_dev, c->st));
+    const bool defer = c->defer_slot >= 0;
+    CUDA_OK(c, mdwf_launch_reduce(0, p, x, p, x, c->L5, c->Vh, c->partial, c->result_dev + (defer ? c->defer_slot : 0), c->st));
     c->launches += 2;
-    return fetch_scalar(c, out);
+    return defer ? MDWF_OK : fetch_scalar(c, out);
 }
 static int v_zero(mdwf_ctx *c, Prec p, const SpinorBuf &x)
 {
@@ -321,9 +324,10 @@ static int finish_norm(mdwf_ctx *c, Prec p, const SpinorBuf &out, bool fused, do
 {
     if (!norm2_out) return MDWF_OK;
     if (!fused) return v_norm2(c, p, out, norm2_out);
-    CUDA_OK(c, mdwf_launch_final_sum(c->hop_partial, (c->Vh + 31) / 32, c->result_dev, c->st));
+    const bool defer = c->defer_slot >= 0;
+    CUDA_OK(c, mdwf_launch_final_sum(c->hop_partial, (c->Vh + 31) / 32, c->result_dev + (defer ? c->defer_slot : 0), c->st));
     c->launches += 1;
-    return fetch_scalar(c, norm2_out);
+    return defer ? MDWF_OK : fetch_scalar(c, norm2_out);
 }
 static int op_Mpc_k2(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out,
                      double *norm2_out = nullptr)
@@ -732,44 +736,68 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
             c->sloppy_applications += 1;
             return MDWF_OK;
         };
+        // The scalars of the iteration stay on the device (result_dev: [1] gamma, [2] ||q||^2, [3] ||r||^2, [4] gamma', [5..8] the
+        // coefficient pairs the BLAS kernels read): alpha and beta are formed by a one-thread kernel, and the host reads back ONE
+        // number per iteration, ||r||^2, for the convergence / reliable-update decision, after it has queued the rest of the
+        // iteration (Mpc^+ r and the x / p update), so the device never waits for it.
+        double *S = c->result_dev, dummy = 0;
+        cudaEvent_t ev;
+        CUDA_OK(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        struct EvGuard { cudaEvent_t e; mdwf_ctx *c; ~EvGuard() { cudaEventDestroy(e); c->defer_slot = -1; mdwf_blas_set_coef(nullptr); } } guard{ev, c};
+        (void)gam;
+        c->defer_slot = 1;                                                  // gamma = ||g||^2
         if (use_bp) {
-            TRY(v_norm2(c, ps, g, &gam));
+            TRY(v_norm2(c, ps, g, &dummy));
+            c->defer_slot = -1;
             TRY(v_zero(c, ps, pc));
             TRY(cg_update(0.0, 0.0));                                       // p = g, B p
         } else {
-            TRY(v_axpby(c, ps, pc, 1.0, ps, g, 0.0, ps, nullptr, &gam));    // p = g, gam = ||g||^2
+            TRY(v_axpby(c, ps, pc, 1.0, ps, g, 0.0, ps, nullptr, &dummy));  // p = g
+            c->defer_slot = -1;
         }
         while (k < maxiter && !converged) {
-            double qq = 0;
-            TRY(apply_Mpc(&qq));
-            if (!(qq > 0.0) || !(gam > 0.0)) break;
-            const double a = gam / qq;
-            TRY(v_axpby(c, ps, rs, -a, ps, q, 1.0, ps, &rs, &r2));          // r -= a q, ||r||^2
+            c->defer_slot = 2;
+            TRY(apply_Mpc(&dummy));                                         // q = Mpc p, ||q||^2
+            CUDA_OK(c, mdwf_launch_cg_scalars(S, 0, c->st));                // alpha = gamma / ||q||^2
+            c->defer_slot = 3;
+            mdwf_blas_set_coef(S + 5);
+            TRY(v_axpby(c, ps, rs, -1.0, ps, q, 1.0, ps, &rs, &dummy));     // r -= alpha q, ||r||^2
+            mdwf_blas_set_coef(nullptr);
+            CUDA_OK(c, cudaMemcpyAsync(c->result_host + 1, S + 3, sizeof(double), cudaMemcpyDeviceToHost, c->st));
+            CUDA_OK(c, cudaEventRecord(ev, c->st));
+            c->defer_slot = 4;
+            TRY(opMdag(ps, rs, ts, g, &dummy));                             // g = Mpc^+ r, gamma' = ||g||^2
+            c->defer_slot = -1;
+            CUDA_OK(c, mdwf_launch_cg_scalars(S, 1, c->st));                // beta = gamma' / gamma, gamma = gamma'
+            mdwf_blas_set_coef(S + 7);
+            TRY(cg_update(1.0, 1.0));                                       // x_lo += alpha p ; p = g + beta p
+            mdwf_blas_set_coef(nullptr);
+            c->launches += 2;
+            CUDA_OK(c, cudaEventSynchronize(ev));
+            r2 = c->result_host[1];
             k++; since_update++;
+            if (!(r2 == r2) || !(r2 >= 0.0)) break;                         // breakdown (gamma or ||q||^2 vanished)
             rn = std::sqrt(r2);
             const bool update = (rn < c->delta * rmax) || (rn <= target) ||
                                 (c->max_update_interval > 0 && since_update >= c->max_update_interval);
-            double gam_new = 0;
             if (update) {
-                // reliable update: fold x_lo into x_hi and recompute the true residual in fp64
-                TRY(v_axpby(c, pxl, xlo, a, ps, pc, 1.0, pxl, &xlo, nullptr));  // x_lo += a p
+                // reliable update: fold x_lo into x_hi, recompute the residual in fp64 and restart the sloppy residual from it
                 TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
                 TRY(v_zero(c, pxl, xlo));
                 TRY(opM(PDd, xhi, te, rhi, nullptr));
-                TRY(v_axpby(c, PDd, rhi, 1.0, PDd, bp, -1.0, PDd, &rhi, &r2));   // r_hi = b' - Mpc x_hi
+                TRY(v_axpby(c, PDd, rhi, 1.0, PDd, bp, -1.0, PDd, &rhi, &r2));   // r_hi = b' - M x_hi
                 rn = std::sqrt(r2);
                 c->reliable_updates += 1;
                 since_update = 0;
                 if (rn <= target) { converged = true; break; }
                 TRY(v_axpby(c, ps, rs, 1.0, PDd, rhi, 0.0, PDd, nullptr, nullptr));
                 rmax = rn;
-                TRY(opMdag(ps, rs, ts, g, &gam_new));                       // g = Mpc^+ r, ||g||^2 fused
-                TRY(cg_update(0.0, gam_new / gam));                         // p = g + (gam'/gam) p   (x_lo is zero)
-            } else {
-                TRY(opMdag(ps, rs, ts, g, &gam_new));
-                TRY(cg_update(a, gam_new / gam));                           // x_lo += a p ; p = g + (gam'/gam) p
+                // the search direction p_{k+1} = g_{k+1} + beta p_k is already built (from the recursive residual, which the true
+                // one replaces to within the sloppy rounding): keep it, and take gamma from the true residual
+                c->defer_slot = 1;
+                TRY(opMdag(ps, rs, ts, g, &dummy));                         // g = Mpc^+ r, gamma = ||g||^2
+                c->defer_slot = -1;
             }
-            gam = gam_new;
         }
         if (!converged) {   // fold what we have
             TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
@@ -877,6 +905,39 @@ int mdwf_wall_project(mdwf_ctx *c, const void *psi_dev, void *q_dev, int real_by
     const int sm = midpoint ? c->L5 / 2 : 0, sp = midpoint ? c->L5 / 2 - 1 : c->L5 - 1;
     CUDA_OK(c, mdwf_launch_wall_project(psi_dev, q_dev, real_bytes, 2L * c->Vh, sm, sp, c->st));
     c->launches += 1;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
+}
+
+// ---- NEXT-4: gradient-flow smearing of the gauge field (Sec. III; App. D) ------------------
+int mdwf_plaquette(mdwf_ctx *c, const void *U_dev, double *out)
+{
+    if (!c || !U_dev || !out) return MDWF_EARG;
+    const long V4 = 2L * c->Vh;
+    const int nb = mdwf_flow_plaquette_blocks(V4);
+    void *part = nullptr;
+    TRY(get_raw(c, "flow.part", sizeof(double) * (size_t)nb, &part));
+    TRY(ensure_scalars(c));
+    CUDA_OK(c, mdwf_launch_plaquette(U_dev, c->L, (double *)part, c->st));
+    CUDA_OK(c, mdwf_launch_final_sum((double *)part, nb, c->result_dev, c->st));
+    c->launches += 2;
+    double s = 0;
+    TRY(fetch_scalar(c, &s));
+    *out = s / (18.0 * (double)V4);                  // <Re tr P> / 3 over the 6 planes
+    return MDWF_OK;
+}
+int mdwf_gradient_flow(mdwf_ctx *c, void *U_dev, double eps, int nsteps, int action, double *plaq_out)
+{
+    if (!c || !U_dev || !(eps > 0.0) || nsteps < 0 || action < 0 || action > 1) return MDWF_EARG;
+    const long V4 = 2L * c->Vh;
+    void *Z = nullptr;
+    TRY(get_raw(c, "flow.z", (size_t)V4 * 4 * 18 * sizeof(double), &Z));
+    const double c0 = action ? 5.0 / 3.0 : 1.0, c1 = action ? -1.0 / 12.0 : 0.0;
+    for (int k = 0; k < nsteps; k++) {
+        CUDA_OK(c, mdwf_launch_flow_step(U_dev, Z, c->L, eps, c0, c1, c->st));
+        c->launches += 6;
+    }
+    if (plaq_out) return mdwf_plaquette(c, U_dev, plaq_out);
     CUDA_OK(c, cudaStreamSynchronize(c->st));
     return MDWF_OK;
 }

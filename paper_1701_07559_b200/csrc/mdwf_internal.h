@@ -112,6 +112,9 @@ int mdwf_launch_xpupdate(Prec px, const SpinorBuf &x, double a, Prec pp, const S
 int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g,
                            const SpinorBuf &pnew, const SpinorBuf &bp, double b5, double c5, double mf, int L5, int Vh,
                            cudaStream_t st);
+// device-resident CG scalars (blas_kernels.cu)
+void mdwf_blas_set_coef(const double *coef_dev);
+int mdwf_launch_cg_scalars(double *S, int mode, cudaStream_t st);
 int mdwf_reduce_max_blocks();
 // fixed-order sum of n partials into *result_dev (second pass of every reduction)
 int mdwf_launch_final_sum(const double *partial, int n, double *result_dev, cudaStream_t st);
@@ -142,6 +145,11 @@ int mdwf_launch_half_import(const void *words, const void *scales, const SpinorB
 // 4D <-> 5D maps on canonical buffers (NEXT-3): wall source injection, wall / midpoint projection
 int mdwf_launch_wall_inject(const void *eta, void *b, int real_bytes, long V4, int L5, cudaStream_t st);
 int mdwf_launch_wall_project(const void *psi, void *q, int real_bytes, long V4, int sm, int sp, cudaStream_t st);
+
+// gradient flow of the gauge field (flow_kernels.cu, NEXT-4): one RK3 step in place; plaquette sum as per-block partials
+int mdwf_launch_flow_step(void *U, void *Z, const int *L, double eps, double c0, double c1, cudaStream_t st);
+int mdwf_launch_plaquette(const void *U, const int *L, double *partial, cudaStream_t st);
+int mdwf_flow_plaquette_blocks(long V4);
 
 // deterministic pseudo-random fill in [-1,1] (timing inputs only)
 int mdwf_launch_fill(Prec p, const SpinorBuf &dst, int L5, int Vh, unsigned seed, cudaStream_t st);

@@ -59,3 +59,25 @@ def test_wall_maps(name, prec):
         got = m.wall_project(psi, midpoint=mid).cpu().numpy().astype(np.complex128)
         assert rel(got, ref) < 1e-7
     m.close()
+
+
+@pytest.mark.parametrize("action", ["wilson", "symanzik"])
+@pytest.mark.parametrize("L", [(4, 4, 4, 6), (6, 4, 2, 8), (2, 2, 4, 4)])
+def test_gradient_flow_parity(action, L):
+    """NEXT-4: the flowed links against the oracle, element by element (fp64), and the mean plaquette"""
+    from oracle import flow_oracle as fo
+    from paper_1701_07559_b200 import binding, inputs
+    if min(L) < 4 and action == "symanzik":
+        pytest.skip("2 x 1 rectangles wrap onto themselves on an extent of 2: the oracle's loop list assumes extents >= 3")
+    U = inputs.gauge_field(L, 0.4, 31)
+    m = binding.Mdwf(L, 8, 1.3, 1.5, 0.5, 0.05)
+    Ud = U.cuda().contiguous()
+    p0 = m.plaquette(Ud)
+    assert abs(p0 - fo.mean_plaquette(U.numpy())) < 1e-13
+    act = fo.WILSON if action == "wilson" else fo.SYMANZIK
+    ref = fo.flow(U.numpy(), 0.03, 3, *act)
+    p1 = m.gradient_flow(Ud, 0.03, 3, action)
+    got = Ud.cpu().numpy()
+    assert np.max(np.abs(got - ref)) < 1e-12
+    assert abs(p1 - fo.mean_plaquette(ref)) < 1e-13 and p1 > p0
+    m.close()
