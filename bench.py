@@ -203,7 +203,13 @@ def main():
     for kv in args.opt:
         m.set_option(*kv.split("=", 1))
     m.load_gauge(U)
+    # the library keeps its own copies of the links; the canonical field goes back to the host (configs[4] needs the memory)
+    want_cpu = rank == 0 and world == 1 and not args.no_cpu_baseline
+    U_host = U.cpu().numpy() if want_cpu else None
+    del U
+    torch.cuda.empty_cache()
     F = m.flops_per_site()
+    torch.cuda.empty_cache()          # hand the generators' temporaries back: the library allocates with cudaMalloc
     sol = torch.empty_like(src)
     tol, maxiter = 1e-10, 100000
 
@@ -258,6 +264,9 @@ def main():
     nbytes = src_h.numel() * 16 * len(srcs)
 
     # ---- per-kernel Dslash numbers and the roofline of the dominant kernel -------------------------------------
+    del srcs, src, sol
+    m.set_option("release_workspace", "1")     # the solver's vectors make room for the timing vectors (configs[4]: 157 GB in use)
+    torch.cuda.empty_cache()
     gl = {18: {"fp64": 8, "fp32": 4, "half": 2}, 12: {"fp64": 8, "fp32": 4, "half": 2}}
     recon = int(cfg["reconstruct"])
     mpc = {}
@@ -265,6 +274,7 @@ def main():
         # two-pass algorithmic bytes per odd 5D site: K1 reads psi, writes t; K2 reads t, psi,
         # writes out (5 spinor streams) + 2 hops x 8 links x recon reals / L5 (+ one fp32 scale per 16-bit spinor)
         b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
+        m.set_option("release_workspace", "1")
         for op, name in ((binding.OP_MPC, "Mpc"), (binding.OP_MPCDAG, "Mpcdag")):
             r = m.time_op(op, prec, reps=args.op_reps, warmup=3)
             mpc["%s_%s" % (name, prec)] = {
@@ -336,18 +346,19 @@ def main():
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nts = min(L[3], args.ref_tslices)
-        r = oracle_sample(cfg, U.cpu().numpy(), src_h.numpy(), nts)
+        r = oracle_sample(cfg, U_host, src_h.numpy(), nts)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
         # the oracle's time for the operator work of one CG iteration on the whole lattice, EXTRAPOLATED from the sample,
         # and for the whole solve at the GPU's iteration count (BLAS-1 not included): context, labelled as extrapolated
         per_it = r["seconds_per_pass"] * L[3] / nts
+        n_rhs = 12 if cfg["source"] == "point12" else 1
         line["cpu_baseline"]["extrapolated"] = {
             "oracle_seconds_per_cg_iteration": per_it,
-            "oracle_solve_seconds_at_gpu_iterations": per_it * int(iters) * len(srcs),
+            "oracle_solve_seconds_at_gpu_iterations": per_it * int(iters) * n_rhs,
             "note": "sample seconds x (Lt / sampled time slices) x GPU iteration count x right-hand sides; not measured"}
         if args.oracle_solve:
             from oracle import mdwf_oracle as mo
-            orc = mo.MdwfOracle(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], U.cpu().numpy())
+            orc = mo.MdwfOracle(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], U_host)
             t0 = time.perf_counter()
             x_ref, it_ref, res_ref = orc.solve(src_h.numpy(), tol=1e-10)
             line["cpu_baseline"]["oracle_full_solve"] = {"iterations": int(it_ref), "seconds": time.perf_counter() - t0,

@@ -86,6 +86,7 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *   "bp_stream"       "1" (default) | "0": 16-bit Krylov vectors only -- the fused CG update also writes B p, which K1 of
  *                     the next Mpc reads instead of applying B on load.
  *   "sweep_mb"        v2-v4: L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
+ *   "release_workspace"  (any value) free the library's pooled work vectors now; they are reallocated on demand.
  *   "max_update_interval"  force a reliable update at least every n iterations (default "0": only the delta rule).
  *   "matpc"           "asym" (default; the operator Chroma uses) | "sym": Schur system mdwf_solve iterates on.
  *                     sym: Mpc_sym x_o = A^{-1} b'_o with Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B ("significant reduction of

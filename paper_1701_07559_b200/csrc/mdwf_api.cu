@@ -527,6 +527,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
         else { c->err = "kernels must be auto|v2|v3|v4|v5"; return MDWF_EARG; }
     } else if (k == "bp_stream") {
         c->use_bp = atoi(value);
+    } else if (k == "release_workspace") {
+        free_pool(c);                            // pooled work vectors are reallocated on demand
     } else if (k == "tile_l2_mb") {
         c->tile_l2_mb = atoi(value);
     } else if (k == "sweep_mb") {
