@@ -225,6 +225,27 @@ def main():
             its.append(it); trs.append(tr); na += m.stat("op_applications"); sec += m.stat("solve_seconds")
         return max(its), max(trs), na, sec
 
+    # ---- per-kernel Dslash numbers: every kernel timed ALONE, before the solves heat the device into its power cap, because the
+    #      roofline they are compared with (MEASURED_PEAKS.json hbm_gbs) is the burst figure of a copy kernel timed alone ----
+    gl = {18: {"fp64": 8, "fp32": 4, "half": 2}, 12: {"fp64": 8, "fp32": 4, "half": 2}}
+    recon = int(cfg["reconstruct"])
+    mpc = {}
+    for prec, rb, extra in (("fp32", 4, 0), ("half", 2, 4), ("fp64", 8, 0)):
+        # two-pass algorithmic bytes per odd 5D site (SURVEY.md 8(d)): K1 reads psi, writes t; K2 reads t, psi,
+        # writes out (5 spinor streams) + 2 hops x 8 links x recon reals / L5 (+ one fp32 scale per 16-bit spinor)
+        b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
+        m.set_option("release_workspace", "1")
+        for op, name in ((binding.OP_MPC, "Mpc"), (binding.OP_MPCDAG, "Mpcdag")):
+            r = m.time_op(op, prec, reps=args.op_reps, warmup=3)
+            mpc["%s_%s" % (name, prec)] = {
+                "ms": r["ms"], "ms_k1": r["ms_k1"], "ms_k2": r["ms_k2"],
+                "tflops": F * h / (r["ms"] * 1e-3) / 1e12,
+                "GBs_model": b_site * h / (r["ms"] * 1e-3) / 1e9,
+                "frac_hbm": b_site * h / (r["ms"] * 1e-3) / 1e9 / hbm_peak,
+                "bytes_per_site_model": b_site}
+    m.set_option("release_workspace", "1")     # the timing vectors make room for the solver's (configs[4]: 157 GB in use)
+    torch.cuda.empty_cache()
+
     # ---- device-resident steps -----------------------------------------------------------------------------
     for _ in range(args.warmup):
         one_solve()
@@ -263,26 +284,8 @@ def main():
     e2e_value = apps_e_all * F * h / e2e_s_max / 1e12
     nbytes = src_h.numel() * 16 * len(srcs)
 
-    # ---- per-kernel Dslash numbers and the roofline of the dominant kernel -------------------------------------
-    del srcs, src, sol
-    m.set_option("release_workspace", "1")     # the solver's vectors make room for the timing vectors (configs[4]: 157 GB in use)
-    torch.cuda.empty_cache()
-    gl = {18: {"fp64": 8, "fp32": 4, "half": 2}, 12: {"fp64": 8, "fp32": 4, "half": 2}}
+    # ---- the roofline of the dominant kernel (per-kernel timings: taken before the solves, see above) ------------------
     recon = int(cfg["reconstruct"])
-    mpc = {}
-    for prec, rb, extra in (("fp64", 8, 0), ("fp32", 4, 0), ("half", 2, 4)):
-        # two-pass algorithmic bytes per odd 5D site (SURVEY.md 8(d)): K1 reads psi, writes t; K2 reads t, psi,
-        # writes out (5 spinor streams) + 2 hops x 8 links x recon reals / L5 (+ one fp32 scale per 16-bit spinor)
-        b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
-        m.set_option("release_workspace", "1")
-        for op, name in ((binding.OP_MPC, "Mpc"), (binding.OP_MPCDAG, "Mpcdag")):
-            r = m.time_op(op, prec, reps=args.op_reps, warmup=3)
-            mpc["%s_%s" % (name, prec)] = {
-                "ms": r["ms"], "ms_k1": r["ms_k1"], "ms_k2": r["ms_k2"],
-                "tflops": F * h / (r["ms"] * 1e-3) / 1e12,
-                "GBs_model": b_site * h / (r["ms"] * 1e-3) / 1e9,
-                "frac_hbm": b_site * h / (r["ms"] * 1e-3) / 1e9 / hbm_peak,
-                "bytes_per_site_model": b_site}
     sloppy = {"d": "fp64", "ds": "fp32", "dh": "half", "dsh": "half"}[cfg["ladder"]]
     rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[sloppy]
     # the four hop kernels of one CG iteration in the sloppy precision; the roofline object describes the slowest

@@ -764,7 +764,7 @@ static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
 // number of neighbour groups the copy engine stages for this launch (0 when the geometry does not allow it)
 template <class P> static inline int hop3_staged(const HopArgs &a)
 {
-    if (a.kver < 4) return 0;                                    // option kernels=v3: every direction through registers
+    if (a.kver != 4) return 0;                                   // only option kernels=v4 stages neighbour groups; v3 and the fall-backs of the tile sweep: every direction through registers
     const long plane = (long)(a.L[0] >> 1) * a.L[1];
     if (plane % 32 != 0 || a.Vh % 32 != 0) return 0;             // groups must not straddle (z,t) planes
     if (a.L[2] < 2 || a.L[3] < 2) return 0;
