@@ -272,6 +272,9 @@ def main():
     srcs_h = [x.cpu().pin_memory() for x in srcs]
     src_h = srcs_h[0]
     sol_h = torch.empty_like(src_h).pin_memory()
+    n_rhs = len(srcs)
+    del srcs, src, sol                 # the host arm stages through the library's own device buffers (configs[4]: 2 x 24.5 GB)
+    torch.cuda.empty_cache()
     one_solve(True, srcs_h, sol_h)
     barrier()
     t0 = time.perf_counter()
@@ -282,7 +285,7 @@ def main():
     e2e_s = time.perf_counter() - t0
     apps_e_all, e2e_s_max = replicas.aggregate(apps_e, e2e_s, device="cuda")
     e2e_value = apps_e_all * F * h / e2e_s_max / 1e12
-    nbytes = src_h.numel() * 16 * len(srcs)
+    nbytes = src_h.numel() * 16 * n_rhs
 
     # ---- the roofline of the dominant kernel (per-kernel timings: taken before the solves, see above) ------------------
     recon = int(cfg["reconstruct"])
@@ -354,7 +357,6 @@ def main():
         # the oracle's time for the operator work of one CG iteration on the whole lattice, EXTRAPOLATED from the sample,
         # and for the whole solve at the GPU's iteration count (BLAS-1 not included): context, labelled as extrapolated
         per_it = r["seconds_per_pass"] * L[3] / nts
-        n_rhs = 12 if cfg["source"] == "point12" else 1
         line["cpu_baseline"]["extrapolated"] = {
             "oracle_seconds_per_cg_iteration": per_it,
             "oracle_solve_seconds_at_gpu_iterations": per_it * int(iters) * n_rhs,

@@ -438,6 +438,10 @@ static int op_Ainv(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &ou
 
 static int op_Ainv_dag(mdwf_ctx *c, Prec p, const SpinorBuf &in, const SpinorBuf &out)
 {
+    if (std::fabs(c->beta / c->alpha) < 0.98) {          // recurrence form (fp32 arithmetic); else the dense table
+        const int rc = mdwf_launch_srec(p, c->L5, c->Vh, in, out, 1, c->alpha, c->beta, c->mf, c->st);
+        if (rc != -1) { CUDA_OK(c, rc); c->launches += 1; return MDWF_OK; }
+    }
     CUDA_OK(c, mdwf_launch_sdense(p, c->L5, c->Vh, in, out, dense_ptr(c, p, DENSE_AINV_DAG), c->st));
     c->launches += 1;
     return MDWF_OK;

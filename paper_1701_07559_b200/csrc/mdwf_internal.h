@@ -98,6 +98,10 @@ int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &
 int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, const void *dense,
                        cudaStream_t st);
 
+// A^{-1} / A^{-dagger} as a recurrence for fp32 arithmetic (s5_kernels.cu); -1 when not covered (fp64, L5 outside {8,12,16}, in == out)
+int mdwf_launch_srec(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, int dag, double alpha, double beta, double mf,
+                     cudaStream_t st);
+
 // BLAS-1 on parity vectors: out = a x + b y (y may be null when b == 0); if partial != nullptr also the
 // deterministic reduction ||out||^2 -> *result_dev (double).  Mixed precisions allowed.
 int mdwf_launch_axpby(Prec po, const SpinorBuf &out, double a, Prec px, const SpinorBuf &x, double b, Prec py,
