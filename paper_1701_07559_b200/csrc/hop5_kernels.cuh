@@ -602,6 +602,15 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------------------
+static inline int mdwf_sm_count()
+{
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    }
+    return sms;
+}
 static inline bool hop5_geometry(HopArgs &a)
 {
     const int Lxh = a.L[0] >> 1;
@@ -654,7 +663,7 @@ template <class P>
 static int launch_hop5_prec(int dag, int pre, int post, int own, HopArgs a, cudaStream_t st)
 {
     if (!hop5_geometry(a)) return -1;
-    if (a.kver == 5 && a.t5_ntiles < 8 * 148) return -1;     // default (auto): a persistent CTA per SM needs several tiles per SM to pay; "kernels=v5" forces it
+    if (a.kver == 5 && a.t5_ntiles < 8 * mdwf_sm_count()) return -1;     // default (auto): a persistent CTA per SM needs several tiles per SM to pay; "kernels=v5" forces it
     if (!dag && pre == 0 && post == 0 && own == 2) return launch_hop5_l5<P, 0, 0, 0, 2>(a, st);   // K2
     if (!dag && pre == 0 && post == 1 && own == 0) return launch_hop5_l5<P, 0, 0, 1, 0>(a, st);   // K1 reading a precomputed B psi
     if (dag && pre == 0 && post == 1 && own == 0) return launch_hop5_l5<P, 1, 0, 1, 0>(a, st);    // K1^+

@@ -11,7 +11,7 @@ from test_gpu_parity import CASES, TOL, setup, to_dev
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("name", ["cfg1", "ragged", "l5_12", "lx32", "l5_24", "kappa1"])
+@pytest.mark.parametrize("name", ["cfg1", "ragged", "l5_12", "l5_16", "lx32", "l5_24", "kappa1", "tile16"])
 @pytest.mark.parametrize("prec", ["fp64", "fp32", "half"])
 def test_symmetric_operator_parity(name, prec):
     from paper_1701_07559_b200 import binding
