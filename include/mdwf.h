@@ -77,15 +77,15 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *   "reliable_delta"  reliable-update threshold delta (default "0.1").
  *   "stream"          cudaStream_t as a decimal integer (default "0").
  *   "kernels"         "auto" (default: v5 where it applies and the lattice has at least 8 tiles per SM, else v3) | "v5" | "v3" |
- *                     "v4" | "v2": kernel family for fp32 arithmetic.  v5: the tile-sweep kernels of
- *                     hop5_kernels.cuh (TMA ring, tensor-memory links and slice history) for K2, K1^dagger, K2^dagger and K1 from
- *                     a precomputed B psi in fp32 storage when Lx/2 in {2,4,8,16}, Ly a multiple of 32/(Lx/2), L5 in {8,12};
- *                     everything else as v3.  v3: hop3_kernels.cuh (link tile by TMA, spinors through registers); v4: v3 with the
- *                     t+- neighbour groups staged by TMA; v2: hop_kernels.cuh (always used for fp64 and other L5).
+ *                     "v2": kernel family for fp32 arithmetic.  v5: the tile-sweep kernels of hop5_kernels.cuh (TMA ring,
+ *                     tensor-memory links and slice history) for K2, K1^dagger, K2^dagger and K1 from a precomputed B psi in fp32
+ *                     storage when Lx/2 in {2,4,8,16}, Ly a multiple of 32/(Lx/2), L5 in {8,12}; everything else as v3.
+ *                     v3: hop3_kernels.cuh (link tile by TMA, spinors through registers; L5 in {8,12,16});
+ *                     v2: hop_kernels.cuh (always used for fp64 and other L5).
  *   "tile_l2_mb"      v5: L2 budget in MB for the working set of a z-chunk of tiles (default 48).
  *   "bp_stream"       "1" (default) | "0": 16-bit Krylov vectors only -- the fused CG update also writes B p, which K1 of
  *                     the next Mpc reads instead of applying B on load.
- *   "sweep_mb"        v2-v4: L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
+ *   "sweep_mb"        v2, v3: L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
  *   "release_workspace"  (any value) free the library's pooled work vectors now; they are reallocated on demand.
  *   "max_update_interval"  force a reliable update at least every n iterations (default "0": only the delta rule).
  *   "matpc"           "asym" (default; the operator Chroma uses) | "sym": Schur system mdwf_solve iterates on.

@@ -586,32 +586,23 @@ MDWF_DEV void bulk_prefetch_l2(const void *src_gmem, unsigned bytes)
 }
 MDWF_DEV unsigned fdiv(unsigned n, const FastDiv &f) { return f.m ? (__umulhi(n, f.m) >> f.s) : n; }
 
-// NST = number of neighbour groups STAGED IN SHARED MEMORY BY THE TMA ENGINE (0, 2: t+-, 4: z+- and t+-).
-// Why (profiles/r02_l2_sm_ceiling.md): L2 delivers 34 TB/s to LDG and >= 22 TB/s to bulk copies on this B200, so the
-// ~10 TB/s the all-LDG kernel pulls is not a delivery cap -- 8 warps of ~250 registers cannot keep more than ~70 KB of
-// loads in flight per SM.  The z+- / t+- neighbours of a 32-site group are whole groups (one contiguous
-// L5*NV*512 B slab each, same lane), nothing else on the SM reuses them, and the block's shared memory is otherwise
-// idle: one elected thread starts their bulk copies (cp.async.bulk, completion on an mbarrier) before the links are
-// staged, the x / y directions stream through registers and L1 as before, and by the time the block reaches the
-// staged directions their data is in shared memory.  Bytes in flight per SM: registers + NST * 37 KB per block.
-template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S, int NST>
+template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
 __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S) > 0 ? Hop3Cfg<P, S>::WARPS / (L5 / S) : 1) hop3_kernel(const HopArgs a)
 {
     constexpr int NSG = L5 / S, NV = P::NV;
     using V = typename P::V;
-    constexpr unsigned BUF_BYTES = L5 * NV * 32 * sizeof(V);          // one staged group
+    constexpr unsigned BUF_BYTES = L5 * NV * 32 * sizeof(V);          // all slices of one 32-site group
     constexpr unsigned NRM_BYTES = P::HALF ? L5 * 32 * sizeof(float) : 0;
-    constexpr unsigned SLOT_BYTES = BUF_BYTES + NRM_BYTES;
     constexpr unsigned SE_BYTES = (POST != 0) ? NSG * 12 * 32 * sizeof(c2) : 0;
     using G = typename P::G;
     constexpr unsigned SL_BYTES = 8 * 9 * 32 * sizeof(float2);
     constexpr unsigned SR_BYTES = P::HALF ? 8 * 9 * 32 * sizeof(short2) : 0;
     extern __shared__ __align__(128) unsigned char smem_raw3[];
-    unsigned char *rest = smem_raw3 + NST * SLOT_BYTES;                // staged groups first (128-byte aligned slabs)
+    unsigned char *rest = smem_raw3;
     c2 *sE = reinterpret_cast<c2 *>(rest);                             // [NSG][12][32] carries / halo slices (POST != 0)
     float2 *sL = reinterpret_cast<float2 *>(rest + SE_BYTES);          // [8][9][32] link table
     unsigned char *sR = rest + SE_BYTES + SL_BYTES;                    // 16-bit storage: the raw link tile
-    unsigned long long *bar = reinterpret_cast<unsigned long long *>(sR + SR_BYTES);   // [1 + NST]: link tile, staged groups
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(sR + SR_BYTES);   // completion of the link tile's bulk copy
     const int lane = threadIdx.x, sg = threadIdx.y, s0 = sg * S;
     const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
     const long sy = Lxh, sz = (long)Lxh * Ly, st = (long)Lxh * Ly * Lz;
@@ -624,10 +615,9 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
     const long cb = cb0 + lane;
     const bool active = cb < a.Vh;
 
-    // ---- one elected thread starts the bulk copies: the link tile of the 32 sites, then the staged neighbour groups ----
+    // ---- one elected thread starts the bulk copy of the link tile of the block's 32 sites (and pulls the own-site slab into L2) ----
     if (lane == 0 && sg == 0) {
-#pragma unroll
-        for (int k = 0; k < 1 + NST; k++) mbar_init(&bar[k], 1);
+        mbar_init(&bar[0], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         const int NK = a.recon >> 1;
@@ -642,25 +632,6 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
         if (OWN != 0) {     // the own-site slab the epilogue reads: pull it into L2 now
             bulk_prefetch_l2(reinterpret_cast<const V *>(a.own) + (cb0 >> 5) * (long)(L5 * NV * 32), BUF_BYTES);
             if (P::HALF) bulk_prefetch_l2(a.own_norm + (cb0 >> 5) * (long)(L5 * 32), NRM_BYTES);
-        }
-        if (NST > 0) {
-            // the launcher guarantees Lxh*Ly % 32 == 0: all 32 sites of the block share (z,t) and their z / t neighbours
-            // are the whole groups at cb0 -+ sz, cb0 -+ st (periodic wrap), lane for lane
-            const unsigned zt = fdiv(fdiv((unsigned)cb0, a.dLxh), a.dLy), t0 = fdiv(zt, a.dLz), z0 = zt - t0 * Lz;
-            long src[4];
-            src[NST - 2] = (t0 == Lt - 1) ? cb0 - (Lt - 1) * st : cb0 + st;
-            src[NST - 1] = (t0 == 0) ? cb0 + (Lt - 1) * st : cb0 - st;
-            if (NST == 4) {
-                src[0] = (z0 == Lz - 1) ? cb0 - (Lz - 1) * sz : cb0 + sz;
-                src[1] = (z0 == 0) ? cb0 + (Lz - 1) * sz : cb0 - sz;
-            }
-#pragma unroll
-            for (int k = 0; k < NST; k++) {
-                unsigned char *dst = smem_raw3 + k * SLOT_BYTES;
-                mbar_expect_tx(&bar[1 + k], SLOT_BYTES);
-                bulk_g2s(dst, reinterpret_cast<const V *>(a.in) + (src[k] >> 5) * (long)(L5 * NV * 32), BUF_BYTES, &bar[1 + k]);
-                if (P::HALF) bulk_g2s(dst + BUF_BYTES, a.in_norm + (src[k] >> 5) * (long)(L5 * 32), NRM_BYTES, &bar[1 + k]);
-            }
         }
     }
 
@@ -708,75 +679,38 @@ __global__ void __launch_bounds__(32 * (L5 / S), Hop3Cfg<P, S>::WARPS / (L5 / S)
 #define MDWF_GDIR(MU, FWD, TD, d, bs) \
         hop_dir3<P, MU, FWD, DAG, PRE, S, TD>(a, L5, s0, sL + (d) * 288 + lane, \
             SrcMem<P, S, true>{gin + sp_off(L5, NV, nb[d], 0), a.in_norm + sp_noff(L5, nb[d], 0), s0, sm, sp}, bs, acc)
-        // neighbour group staged in slot k: same lane
-#define MDWF_SDIR(MU, FWD, TD, d, bs, k) \
-        do { mbar_wait(&bar[1 + (k)], 0); \
-             hop_dir3<P, MU, FWD, DAG, PRE, S, TD>(a, L5, s0, sL + (d) * 288 + lane, \
-                 SrcMem<P, S, false>{reinterpret_cast<const V *>(smem_raw3 + (k) * SLOT_BYTES) + lane, \
-                                     reinterpret_cast<const float *>(smem_raw3 + (k) * SLOT_BYTES + BUF_BYTES) + lane, s0, sm, sp}, bs, acc); } while (0)
         if constexpr (EARLY) hop_dir3<P, 0, true, DAG, PRE, S, false>(a, L5, s0, sL + 0 * 288 + lane, first, 1.f, acc);
         else MDWF_GDIR(0, true, false, 0, 1.f);
         MDWF_GDIR(0, false, false, 4, 1.f);
         MDWF_GDIR(1, true, false, 1, 1.f);
         MDWF_GDIR(1, false, false, 5, 1.f);
-        if (NST == 4) {
-            MDWF_SDIR(2, true, false, 2, 1.f, 0);
-            MDWF_SDIR(2, false, false, 6, 1.f, 1);
-        } else {
-            MDWF_GDIR(2, true, false, 2, 1.f);
-            MDWF_GDIR(2, false, false, 6, 1.f);
-        }
-        if (NST >= 2) {
-            MDWF_SDIR(3, true, true, 3, btp, NST - 2);
-            MDWF_SDIR(3, false, true, 7, btm, NST - 1);
-        } else {
-            MDWF_GDIR(3, true, true, 3, btp);
-            MDWF_GDIR(3, false, true, 7, btm);
-        }
+        MDWF_GDIR(2, true, false, 2, 1.f);
+        MDWF_GDIR(2, false, false, 6, 1.f);
+        MDWF_GDIR(3, true, true, 3, btp);
+        MDWF_GDIR(3, false, true, 7, btm);
 #undef MDWF_GDIR
-#undef MDWF_SDIR
     }
 
     epilogue3<P, DAG, POST, OWN, L5, S>(a, acc, sE, lane, sg, s0, cb, active, (int)blockIdx.x);
 }
 
 // ---- launchers ----------------------------------------------------------------------------------
-template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S, int NST>
-static int launch_hop3_inst(const HopArgs &a, cudaStream_t st)
-{
-    constexpr int NSG = L5 / S;
-    using V = typename P::V;
-    dim3 block(32, NSG);
-    dim3 grid((unsigned)((a.Vh + 31) / 32));
-    const size_t smem = (size_t)NST * ((size_t)L5 * P::NV * 32 * sizeof(V) + (P::HALF ? (size_t)L5 * 32 * sizeof(float) : 0)) +
-                        ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float2) +
-                        (P::HALF ? (size_t)8 * 9 * 32 * sizeof(short2) : 0) + 8 * (1 + NST);
-    static bool attr_set = false;                                // once per instantiation, not once per launch
-    if (smem > 32 * 1024 && !attr_set) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
-        cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S, NST>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
-        attr_set = true;
-    }
-    hop3_kernel<P, DAG, PRE, POST, OWN, L5, S, NST><<<grid, block, smem, st>>>(a);
-    return (int)cudaGetLastError();
-}
-// number of neighbour groups the copy engine stages for this launch (0 when the geometry does not allow it)
-template <class P> static inline int hop3_staged(const HopArgs &a)
-{
-    if (a.kver != 4) return 0;                                   // only option kernels=v4 stages neighbour groups; v3 and the fall-backs of the tile sweep: every direction through registers
-    const long plane = (long)(a.L[0] >> 1) * a.L[1];
-    if (plane % 32 != 0 || a.Vh % 32 != 0) return 0;             // groups must not straddle (z,t) planes
-    if (a.L[2] < 2 || a.L[3] < 2) return 0;
-    return P::HALF ? MDWF_H3_NST_H : MDWF_H3_NST_S;
-}
 template <class P, int DAG, int PRE, int POST, int OWN, int L5, int S>
 static int launch_hop3_nst(const HopArgs &a, cudaStream_t st)
 {
-    const int nst = hop3_staged<P>(a);
-    if (nst == 4) return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, (P::HALF ? 4 : 2)>(a, st);   // fp32 slabs: 2 fit beside a second block
-    if (nst == 2) return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, 2>(a, st);
-    return launch_hop3_inst<P, DAG, PRE, POST, OWN, L5, S, 0>(a, st);
+    constexpr int NSG = L5 / S;
+    dim3 block(32, NSG);
+    dim3 grid((unsigned)((a.Vh + 31) / 32));
+    const size_t smem = ((POST != 0) ? (size_t)NSG * 12 * 32 * sizeof(c2) : 0) + (size_t)8 * 9 * 32 * sizeof(float2) +
+                        (P::HALF ? (size_t)8 * 9 * 32 * sizeof(short2) : 0) + 8;
+    static bool attr_set = false;                                // once per instantiation, not once per launch
+    if (smem > 32 * 1024 && !attr_set) {     // dynamic + the kernel's static shared memory must stay under the 48 KB default
+        cudaError_t e = cudaFuncSetAttribute(hop3_kernel<P, DAG, PRE, POST, OWN, L5, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        attr_set = true;
+    }
+    hop3_kernel<P, DAG, PRE, POST, OWN, L5, S><<<grid, block, smem, st>>>(a);
+    return (int)cudaGetLastError();
 }
 template <class P, int DAG, int PRE, int POST, int OWN>
 static int launch_hop3_l5(const HopArgs &a, cudaStream_t st)

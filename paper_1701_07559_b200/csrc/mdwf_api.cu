@@ -527,8 +527,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
     } else if (k == "kernels") {
-        if (v == "auto") c->kver = 5; else if (v == "v5") c->kver = 6; else if (v == "v4") c->kver = 4; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
-        else { c->err = "kernels must be auto|v2|v3|v4|v5"; return MDWF_EARG; }
+        if (v == "auto") c->kver = 5; else if (v == "v5") c->kver = 6; else if (v == "v3") c->kver = 3; else if (v == "v2") c->kver = 2;
+        else { c->err = "kernels must be auto|v2|v3|v5"; return MDWF_EARG; }
     } else if (k == "bp_stream") {
         c->use_bp = atoi(value);
     } else if (k == "release_workspace") {

@@ -20,13 +20,6 @@
 #ifndef MDWF_H3_WARPS_H
 #define MDWF_H3_WARPS_H 12
 #endif
-// neighbour groups staged by the TMA engine in the v3 kernels (0, 2 = t+-, 4 = z+- and t+-), per storage format
-#ifndef MDWF_H3_NST_S
-#define MDWF_H3_NST_S 2
-#endif
-#ifndef MDWF_H3_NST_H
-#define MDWF_H3_NST_H 2
-#endif
 static inline int mdwf_h3_slices(int L5) { return L5 == 12 ? MDWF_H3_S12 : 2; }
 
 enum Prec { PREC_D = 0, PREC_S = 1, PREC_H = 2 };
@@ -76,7 +69,7 @@ struct HopArgs {
     double *partial;         // v3 kernels: if non-null, ||out||^2 partial sums, one per block (fused norm, S7)
     const void *dense;       // POST = 1: device pointer to R[2][L5][L5] (P+ block, then P- block)
     // POST = 1 in the v3 kernels (hop3_kernels.cuh): coef_hop * B A^{-1} as a blocked recurrence
-    int kver;                // host side: kernel family requested (2: hop_kernels.cuh, 3: hop3 all-LDG, 4: hop3 with TMA-staged z/t neighbours, 5: hop5 tile sweep where covered)
+    int kver;                // host side: kernel family requested (2: hop_kernels.cuh, 3: hop3_kernels.cuh, 5: hop5 tile sweep where it pays, 6: hop5 wherever covered)
     int r_ok;                // 1 when the recurrence form is usable (|kappa| < 1)
     float r_nk;              // -kappa = -beta/alpha
     float r_cpow;            // (-kappa)^S, S = slices per thread

@@ -29,7 +29,7 @@ def test_solve_oracle_true_residual(i):
     orc = MdwfOracle(L, L5, cfg["M5"], cfg["b5"], cfg["c5"], cfg["mf"], U.cpu().numpy())
     del U
     if cfg["source"] == "point12":
-        sources = [inputs.point_source(L, L5, sp, col, device="cuda") for sp, col in ((0, 0), (2, 1))]
+        sources = [inputs.point_source(L, L5, sp, col, device="cuda") for sp in range(4) for col in range(3)]   # all 12 columns
     else:
         sources = [inputs.gaussian_source(L, L5, cfg["seed"], device="cuda")]
     for b in sources:

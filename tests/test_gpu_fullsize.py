@@ -1,7 +1,7 @@
 """Parity at BASELINE.json's full size, in the launch configuration bench.py times (configs[3]: 32^3 x 96, L5 = 12,
 12-real links): the CUDA Mpc / Mpc^dagger in fp64, fp32 and 16-bit storage against the oracle evaluated one by
 one on sampled odd sites (corners, all four wrap-arounds incl. the antiperiodic t boundary, and random sites).
-Tolerances: north_star's 1e-12 / 1e-5; 2e-3 for the 16-bit operator."""
+Tolerances: north_star's 1e-12 / 1e-5; 2e-4 for the 16-bit operator."""
 import numpy as np
 import pytest
 import torch
@@ -49,8 +49,9 @@ def test_mpc_sampled_sites_at_config4():
     sites = sample_sites(orc, 48, 7)
     cbs = torch.from_numpy(sites // 2).cuda()
     ref = {binding.OP_MPC: orc.Mpc_at_sites(v_o, sites), binding.OP_MPCDAG: orc.Mpc_at_sites(v_o, sites, dagger=True)}
-    # v3 = default kernels (hop3_kernels.cuh); v4 = neighbours staged by bulk-asynchronous copies (hop4_kernels.cuh)
-    for kern, prec in (("v3", "fp64"), ("v3", "fp32"), ("v3", "half"), ("v4", "fp32"), ("v4", "half")):
+    # auto = what bench.py times: the tile-sweep kernels (hop5_kernels.cuh) for fp32 storage at this size, hop3_kernels.cuh for
+    # K1 and for 16-bit storage, hop_kernels.cuh for fp64; v3 = hop3_kernels.cuh for every fp32 kernel
+    for kern, prec in (("auto", "fp64"), ("auto", "fp32"), ("auto", "half"), ("v3", "fp32")):
         m.set_option("kernels", kern)
         m.set_option("apply_precision", prec)
         x = bo_dev if prec == "fp64" else bo_dev.to(torch.complex64)

@@ -21,7 +21,7 @@ CASES = {
     "l5_12": ((6, 4, 2, 8), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 3),         # several blocks, config-4 parameters
     "l5_16": ((2, 2, 4, 4), 16, 1.3, 1.75, 0.75, 0.00712, 0.2, 5),     # a15m220 row of Table II
     "l5_24": ((2, 2, 2, 4), 24, 1.3, 2.25, 1.25, 0.00216, 0.2, 6),     # a15m130 row of Table II (generic path)
-    "lx32": ((32, 4, 2, 4), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 7),         # Lx = 32: the geometry the v4 (staged) kernels cover
+    "lx32": ((32, 4, 2, 4), 12, 1.1, 1.5, 0.5, 0.005, 0.1, 7),         # Lx = 32, Lz = 2: tile sweep with the z halo wrapping onto the tile
     "tile8": ((8, 8, 4, 4), 8, 1.2, 1.25, 0.25, 0.01, 0.2, 21),          # v5 tile sweep: Lx/2 = 4, 8 rows per group, one group in y, L5 = 8
     "tile16": ((16, 4, 4, 6), 12, 1.3, 1.75, 0.75, 0.02, 0.2, 22),       # v5 tile sweep: Lx/2 = 8, 4 rows per group, Lt/2 odd
     "l5_2": ((2, 2, 2, 2), 2, 1.3, 1.5, 0.5, 0.05, 0.3, 12),           # smallest lattice and smallest L5 the ABI accepts
@@ -73,9 +73,9 @@ def test_operator_parity(name, prec, recon):
     m.close()
 
 
-@pytest.mark.parametrize("name", ["lx32", "l5_12", "tile8", "tile16"])       # l5_12: v4 / v5 are not applicable and must fall back to v3
+@pytest.mark.parametrize("name", ["lx32", "l5_12", "tile8", "tile16"])       # l5_12: v5 is not applicable and must fall back to v3
 @pytest.mark.parametrize("prec", ["fp32", "half"])
-@pytest.mark.parametrize("kernels", ["v4", "v3", "v5"])
+@pytest.mark.parametrize("kernels", ["v2", "v3", "v5"])
 def test_operator_parity_kernel_families(name, prec, kernels):
     """every selectable kernel family (option kernels=...), incl. the y wrap-around at Ly = 4; the default is v5"""
     from paper_1701_07559_b200 import binding

@@ -35,7 +35,7 @@ def test_create_validates_arguments(binding):
     for k, v in (("ladder", "dsh"), ("reconstruct", "12"), ("apply_precision", "half"), ("reliable_delta", "0.2"),
                  ("matpc", "asym"), ("matpc", "sym"), ("kernels", "auto"), ("kernels", "v5"), ("tile_l2_mb", "64")):
         binding.mdwf_set_option(h, k, v)
-    for k, v in (("ladder", "x"), ("reconstruct", "8"), ("matpc", "both"), ("kernels", "v9"), ("nope", "1"), ("reliable_delta", "2")):
+    for k, v in (("ladder", "x"), ("reconstruct", "8"), ("matpc", "both"), ("kernels", "v4"), ("nope", "1"), ("reliable_delta", "2")):
         with pytest.raises(binding.MdwfError):
             binding.mdwf_set_option(h, k, v)
     binding.mdwf_destroy(h)
