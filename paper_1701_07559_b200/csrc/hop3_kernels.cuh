@@ -567,9 +567,9 @@ MDWF_DEV void mbar_wait(unsigned long long *bar, unsigned phase)
     unsigned ok = 0;
     const unsigned addr = smem_u32(bar);
     while (!ok) {
-        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.u32 %0, 1, 0, P1;\n\t}"
+        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, P1;\n\t}"
                      : "=r"(ok)
-                     : "r"(addr), "r"(phase)
+                     : "r"(addr), "r"(phase), "r"(0x989680u)          // suspend-time hint: sleep in hardware rather than poll
                      : "memory");
     }
 }

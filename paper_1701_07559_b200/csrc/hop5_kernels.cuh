@@ -176,9 +176,9 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
     unsigned long long *full = bars, *empty = bars + RING;                          // ring: producer -> sweep, sweep -> producer
     unsigned long long *hfull = bars + 2 * RING, *hempty = hfull + 4 * HIST_SLOTS;   // history: per warp pair, per slot
     unsigned long long *lfree = hempty + 4 * HIST_SLOTS;                             // unused (links ride in the ring)
-    long *ysrc = reinterpret_cast<long *>(lfree + 4);                                // [48] y-halo row table of the producer
-    unsigned *ydst = reinterpret_cast<unsigned *>(ysrc + 48);                        // [48]
-    unsigned *tmem_base_s = ydst + 48;
+    long *ysrc = reinterpret_cast<long *>(lfree + 4);                                // [3][48] y-halo row table, one per helper warp (they may be a tile apart)
+    unsigned *ydst = reinterpret_cast<unsigned *>(ysrc + 3 * 48);                    // [3][48]
+    unsigned *tmem_base_s = ydst + 3 * 48;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int Lxh = a.L[0] >> 1, Ly = a.L[1], Lz = a.L[2], Lt = a.L[3];
     const int NK = a.recon >> 1;
@@ -247,6 +247,8 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
         const int nyu = (8 * NV * Lxh) / 32;                              // copies per lane per slice
         const int xoff = (lane & (Lxh - 1)) * SL::CH, rpw = 32 / Lxh, r0 = lane / Lxh;   // rows per warp instruction, this lane's row
         unsigned it = 0;
+        ysrc += 48 * (warp - 9);
+        ydst += 48 * (warp - 9);
         for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const Tile T = tile_of(a, tile);
             for (int h = 0; h < 2; h++) {                                           // link items: nothing to copy
@@ -637,7 +639,7 @@ template <class P, int DAG, int PRE, int POST, int OWN, int L5>
 static int launch_hop5_inst(const HopArgs &a, cudaStream_t st)
 {
     static int sms = 0;
-    const size_t smem = (size_t)RING * Slot<P>::BYTES + 8 * (2 * RING + 8 * HIST_SLOTS + 4) + 48 * 12 + 16;
+    const size_t smem = (size_t)RING * Slot<P>::BYTES + 8 * (2 * RING + 8 * HIST_SLOTS + 4) + 3 * 48 * 12 + 16;
     if (!sms) {
         int dev = 0;
         cudaGetDevice(&dev);

@@ -20,6 +20,7 @@ int mdwf_launch_hop_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_S(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop3_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_hop5_S(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop6_H(int, int, int, int, const HopArgs &, cudaStream_t);
 int mdwf_launch_sdense_mma(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_D(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
 int mdwf_launch_sdense_S(int, int, const SpinorBuf &, const SpinorBuf &, const void *, cudaStream_t);
@@ -29,6 +30,10 @@ int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &
 {
     if (a.kver >= 5 && p == PREC_S) {        // v5 tile sweep; -1 = not covered, fall back to v3
         const int rc = mdwf_launch_hop5_S(dag, pre, post, own, a, st);
+        if (rc != -1) return rc;
+    }
+    if (a.kver >= 5 && p == PREC_H) {        // tile sweep for 16-bit storage (two sweep sets); -1 = not covered
+        const int rc = mdwf_launch_hop6_H(dag, pre, post, own, a, st);
         if (rc != -1) return rc;
     }
     if (a.kver >= 3 && p != PREC_D) {        // v3 family (fp32 arithmetic); -1 = not covered, fall back to v2
