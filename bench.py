@@ -296,18 +296,27 @@ def main():
     b2 = (3 * (24 * rb + extra) + 8 * recon * rb / L5) * h      # K2 / K2+: read two vectors, write one
     fam = "hop_kernel" if sloppy == "fp64" else "hop3_kernel"
     tiles = (L[1] * (L[0] // 2) // 32) * (L[2] // 2) * (L[3] // 2) if (L[0] // 2) in (2, 4, 8, 16) and (L[1] * (L[0] // 2)) % 32 == 0 else 0
-    fam5 = "hop5_kernel" if (sloppy == "fp32" and L5 in (8, 12) and tiles >= 8 * 148) else fam   # tile-sweep kernels (not for K1 with B on load)
+    swept = L5 in (8, 12) and tiles >= 8 * 148            # the library's rule for the tile-sweep kernels (hop5 / hop6 launchers)
     pname = {"fp64": "PD", "fp32": "PS", "half": "PH"}[sloppy]
     k1b = sloppy == "half"                                      # 16-bit CG: K1 reads the B p stream, no B on load
+
+    def kernel(dag, pre, post, own):
+        # the kernel the library launches for this (precision, variant): mdwf_launch_hop in mdwf_api.cu
+        if sloppy == "fp32" and swept and pre == 0:
+            return "hop5_kernel<PS,%d,0,%d,%d,%d>" % (dag, post, own, L5)
+        if sloppy == "half" and swept and pre == 0 and post != 2:
+            return "hop6_kernel<%d,%d,%d,%d>" % (dag, post, own, L5)      # two sweep sets, 16-bit storage; K2^+ stays on hop3
+        return "%s<%s,%d,%d,%d,%d,%d%s>" % (fam, pname, dag, pre, post, own, L5, ",3" if fam == "hop_kernel" or post == 1 else "")
+
     mp, md = mpc["Mpc_%s" % sloppy], mpc["Mpcdag_%s" % sloppy]
     cands = [
-        ("%s<%s,0,%d,1,0,%d,3> (K1 of Mpc: t_e = B A^-1 H_eo %s)" % (fam, pname, 0 if k1b else 1, L5,
-                                                                  "(B psi)_o, B psi streamed by the CG update" if k1b else "B psi_o"),
+        ("%s (K1 of Mpc: t_e = B A^-1 H_eo %s)" % (kernel(0, 0 if k1b else 1, 1, 0),
+                                                  "(B psi)_o, B psi streamed by the CG update" if k1b else "B psi_o"),
          mp["ms_k1"], b1, 1320 + (0 if k1b else 72) + 72 + 48 * L5 - 24, "k1"),
-        ("%s<%s,0,0,0,2,%d> (K2 of Mpc: A psi_o - 1/4 H_oe t_e)" % (fam5, pname, L5), mp["ms_k2"], b2, 1320 + 72 + 48, "k2"),
-        ("%s<%s,1,0,1,0,%d> (K1 of Mpc^dagger: u_e = A^-+ B^+ H'_eo psi_o)" % (fam5, pname, L5), md["ms_k1"], b1,
+        ("%s (K2 of Mpc: A psi_o - 1/4 H_oe t_e)" % kernel(0, 0, 0, 2), mp["ms_k2"], b2, 1320 + 72 + 48, "k2"),
+        ("%s (K1 of Mpc^dagger: u_e = A^-+ B^+ H'_eo psi_o)" % kernel(1, 0, 1, 0), md["ms_k1"], b1,
          1320 + 72 + 48 * L5 - 24, "k1"),
-        ("%s<%s,1,0,2,3,%d> (K2 of Mpc^dagger: A^+ psi_o - 1/4 B^+ H'_oe u_e)" % (fam5, pname, L5), md["ms_k2"], b2,
+        ("%s (K2 of Mpc^dagger: A^+ psi_o - 1/4 B^+ H'_oe u_e)" % kernel(1, 0, 2, 3), md["ms_k2"], b2,
          1320 + 72 + 72 + 48, "k2"),
     ]
     kname, k_ms, k_bytes, k_flops_site, k_key = max(cands, key=lambda c: c[1])
