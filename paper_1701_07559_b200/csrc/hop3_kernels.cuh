@@ -205,6 +205,47 @@ MDWF_DEV void project3(const c2 *v, c2 *h)
         }
     }
 }
+// ---- spin projection straight from the stored 16-bit words ------------------------------------------------------------
+// 0x4B400000 | u is the float M + q (M = 12615680, q the stored integer; cvt_raw above).  The projected half spinor
+// h = v_a +- v_b (or +- i v_b) is needed as the integers q_a +- q_b, so the magic constant need not be subtracted from each input
+// first: a "-" lane is (M + q_a) - (M + q_b), a "+" lane is (M + q_a) + ((M + q_b) - 2M); every intermediate is an integer below
+// 2^24, so all of it is exact and the result is bit-identical to converting first.  Per projected complex: one FFMA2, plus one
+// FADD2 when it has a "+" lane, instead of two FADD2 and the FFMA2: 84 instead of 144 FMA-pipe instructions per 8 directions.
+MDWF_DEV c2 magic_pair(unsigned w)
+{
+    return mk(__uint_as_float(__byte_perm(w, 0x4B400000u, 0x7610)), __uint_as_float(__byte_perm(w, 0x4B400000u, 0x7632)));
+}
+// (q_a.x + SX q_b[SWAP ? y : x], q_a.y + SY q_b[SWAP ? x : y]) from the magic floats of a and b
+template <int SX, int SY, bool SWAP>
+MDWF_DEV c2 comb(c2 fa, c2 fb)
+{
+    constexpr float M2 = -2.0f * 12615680.0f;
+    constexpr float kx = SWAP ? (SY > 0 ? M2 : 0.f) : (SX > 0 ? M2 : 0.f), ky = SWAP ? (SX > 0 ? M2 : 0.f) : (SY > 0 ? M2 : 0.f);
+    const c2 t = (SX > 0 || SY > 0) ? add2(fb, mk(kx, ky)) : fb;
+    return fma2(SWAP ? swp(t) : t, mk((float)SX, (float)SY), fa);
+}
+// project3 on the magic floats f[spin*3+colour] of a stored spinor: h = the projected integers (same table as project3)
+template <int MU, int SGN>
+MDWF_DEV void project3m(const c2 *f, c2 *h)
+{
+    constexpr int S = SGN;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if (MU == 0) {
+            h[c] = comb<S, -S, true>(f[c], f[9 + c]);
+            h[3 + c] = comb<S, -S, true>(f[3 + c], f[6 + c]);
+        } else if (MU == 1) {
+            h[c] = comb<S, S, false>(f[c], f[9 + c]);
+            h[3 + c] = comb<-S, -S, false>(f[3 + c], f[6 + c]);
+        } else if (MU == 2) {
+            h[c] = comb<S, -S, true>(f[c], f[6 + c]);
+            h[3 + c] = comb<-S, S, true>(f[3 + c], f[9 + c]);
+        } else {
+            h[c] = comb<-S, -S, false>(f[c], f[6 + c]);
+            h[3 + c] = comb<-S, -S, false>(f[3 + c], f[9 + c]);
+        }
+    }
+}
 // acc += sc * [chi ; lower(chi)],  sc = +-1 (antiperiodic t hop), acc[spin*3+colour]
 template <int MU, int SGN, bool WITHSC>
 MDWF_DEV void recon3(const c2 *chi, float sc, c2 *acc)
@@ -309,8 +350,14 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const
             c2 v[12], h[6], chi[6];
             if constexpr (P::HALF) {
                 const float sck = src.scale(k);
-                take<false, 0, 6>(src, k, 1.f, v);
-                project3<MU, SGN>(v, h);
+#pragma unroll
+                for (int j = 0; j < 6; j++) {
+                    const typename P::V q = src.chunk(k, j);
+                    const uint2 w = *reinterpret_cast<const uint2 *>(&q);
+                    v[2 * j] = magic_pair(w.x);
+                    v[2 * j + 1] = magic_pair(w.y);
+                }
+                project3m<MU, SGN>(v, h);
                 su3_mul3(U, h, chi);
                 recon3<MU, SGN, true>(chi, TDIR ? bsign * sck : sck, acc[k]);
             } else {
@@ -352,8 +399,9 @@ MDWF_DEV void hop_dir3(const HopArgs &a, int L5, int s0, const float2 *sl, const
 
 // ---- spinor store from complex pairs ---------------------------------------------------------------
 // returns the sum of squares of the values as stored (for the fused norm of the output vector)
-template <class P> MDWF_DEV float store3(void *base, float *norm, int L5, int s, long cb, const c2 *o);
-template <> MDWF_DEV float store3<PS>(void *base, float *, int L5, int s, long cb, const c2 *o)
+// stores one (site, slice); returns its contribution to the fused norm (of the values as stored) when want_norm is set
+template <class P> MDWF_DEV float store3(void *base, float *norm, int L5, int s, long cb, const c2 *o, bool want_norm = true);
+template <> MDWF_DEV float store3<PS>(void *base, float *, int L5, int s, long cb, const c2 *o, bool)
 {
     float4 *p = reinterpret_cast<float4 *>(base) + sp_off(L5, PS::NV, cb, s);
 #pragma unroll
@@ -363,7 +411,7 @@ template <> MDWF_DEV float store3<PS>(void *base, float *, int L5, int s, long c
     for (int q = 1; q < 12; q++) n2 = fma2(o[q], o[q], n2);
     return n2.x + n2.y;
 }
-template <> MDWF_DEV float store3<PH>(void *base, float *norm, int L5, int s, long cb, const c2 *o)
+template <> MDWF_DEV float store3<PH>(void *base, float *norm, int L5, int s, long cb, const c2 *o, bool want_norm)
 {
     short4 *p = reinterpret_cast<short4 *>(base) + sp_off(L5, PH::NV, cb, s);
     float m = 0.f;
@@ -380,9 +428,11 @@ template <> MDWF_DEV float store3<PH>(void *base, float *norm, int L5, int s, lo
         const c2 e = fma2(o[2 * j], isc, magic), f = fma2(o[2 * j + 1], isc, magic);
         pw[32 * j] = make_uint2(__byte_perm(__float_as_uint(e.x), __float_as_uint(e.y), 0x5410),
                                 __byte_perm(__float_as_uint(f.x), __float_as_uint(f.y), 0x5410));
-        const c2 qe = add2(e, nmagic), qf = add2(f, nmagic);      // the stored integers, exactly
-        n2 = fma2(qe, qe, n2);
-        n2 = fma2(qf, qf, n2);
+        if (want_norm) {                                          // uniform over the kernel: K1 / K1^dagger have no fused norm
+            const c2 qe = add2(e, nmagic), qf = add2(f, nmagic);  // the stored integers, exactly
+            n2 = fma2(qe, qe, n2);
+            n2 = fma2(qf, qf, n2);
+        }
     }
     const float sc = m * (1.0f / MDWF_FIXED_MAX);
     return (n2.x + n2.y) * sc * sc;
@@ -509,29 +559,39 @@ MDWF_DEV void epilogue3(const HopArgs &a, c2 (*acc)[12], c2 *sE, int lane, int s
 #pragma unroll
             for (int q = 0; q < 12; q++) o[q] = fma2(coef2, acc[k][q], w[q]);
         } else {
-            // (own_d + own_o Lambda) psi: upper from s-1, lower from s+1; Lambda^dagger (OWN == 3): swapped
+            // (own_d + own_o Lambda) psi: upper from s-1, lower from s+1; Lambda^dagger (OWN == 3): swapped.
+            // 16-bit storage: the stored integers are used as they are and the scale of each slice goes into its coefficient
             c2 w[12], u[6], l[6];
             const V *p = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, s);
-            Ld<P>::template chunks<12>(p, load_scale<P>(a.own_norm, sp_noff(L5, cb, s)), w);
             int su = (OWN == 2) ? s - 1 : s + 1;
             int sl = (OWN == 2) ? s + 1 : s - 1;
-            float fu = (float)a.own_o, fl = (float)a.own_o;
+            float fu = (float)a.own_o, fl = (float)a.own_o, fd = (float)a.own_d;
             if (su < 0) { su = L5 - 1; fu *= (float)(-a.mf); }
             if (su >= L5) { su = 0; fu *= (float)(-a.mf); }
             if (sl < 0) { sl = L5 - 1; fl *= (float)(-a.mf); }
             if (sl >= L5) { sl = 0; fl *= (float)(-a.mf); }
             const V *pu = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, su);
             const V *pl = reinterpret_cast<const V *>(a.own) + sp_off(L5, P::NV, cb, sl) + 32 * (P::NV / 2);
-            Ld<P>::template chunks<6>(pu, load_scale<P>(a.own_norm, sp_noff(L5, cb, su)), u);
-            Ld<P>::template chunks<6>(pl, load_scale<P>(a.own_norm, sp_noff(L5, cb, sl)), l);
-            const c2 d2 = dup((float)a.own_d), fu2 = dup(fu), fl2 = dup(fl);
+            if constexpr (P::HALF) {
+                Ld<P>::template raw<12>(p, w);
+                Ld<P>::template raw<6>(pu, u);
+                Ld<P>::template raw<6>(pl, l);
+                fd *= load_scale<P>(a.own_norm, sp_noff(L5, cb, s));
+                fu *= load_scale<P>(a.own_norm, sp_noff(L5, cb, su));
+                fl *= load_scale<P>(a.own_norm, sp_noff(L5, cb, sl));
+            } else {
+                Ld<P>::template chunks<12>(p, 1.f, w);
+                Ld<P>::template chunks<6>(pu, 1.f, u);
+                Ld<P>::template chunks<6>(pl, 1.f, l);
+            }
+            const c2 d2 = dup(fd), fu2 = dup(fu), fl2 = dup(fl);
 #pragma unroll
             for (int q = 0; q < 6; q++) {
                 o[q] = fma2(coef2, acc[k][q], fma2(d2, w[q], mul2(fu2, u[q])));
                 o[6 + q] = fma2(coef2, acc[k][6 + q], fma2(d2, w[6 + q], mul2(fl2, l[q])));
             }
         }
-        nsum += store3<P>(a.out, a.out_norm, L5, s, cb, o);
+        nsum += store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
     }
     }
     if (a.partial) {

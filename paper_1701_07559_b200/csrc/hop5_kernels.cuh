@@ -461,7 +461,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
 #pragma unroll
                         for (int q = 0; q < 6; q++) pu[q] = cur[q];
                     }
-                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 }
             }
             if (POST == 1) {
@@ -516,7 +516,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
                         zn[q] = z;
                         o[DOFF / 2 + q] = fma2(qWd, zp[q], x[DOFF / 2 + q]);            // zp = z_{L5-1} of the direct half = its W
                     }
-                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 }
                 hit += L5;
             }
@@ -560,7 +560,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
                         o[q] = fma2(cd2, x[q], fma2(cou, mk(xu[2 * q], xu[2 * q + 1]), fma2(od2, pc[q], mul2(oou, pu[q]))));
                         o[6 + q] = fma2(cd2, x[6 + q], fma2(col, mk(xl[2 * q], xl[2 * q + 1]), fma2(od2, pc[6 + q], mul2(ool, pl[6 + q]))));
                     }
-                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 };
                 MDWF_HWAIT(0);
                 MDWF_HWAIT(1);

@@ -57,18 +57,28 @@ MDWF_DEV float raw_ints(const Raw &b, c2 *v)
     for (int j = 0; j < 6; j++) { v[2 * j] = cvt_raw(b.q[j].x); v[2 * j + 1] = cvt_raw(b.q[j].y); }
     return b.sc * (1.0f / MDWF_FIXED_MAX);
 }
-// values of the upper (half = 0) or lower (half = 1) six complex numbers
+// spin projection straight from the stored words (project3m, hop3_kernels.cuh)
+template <int MU, int SGN>
+MDWF_DEV void project_magic(const Raw &b, c2 *h)
+{
+    c2 f[12];
+#pragma unroll
+    for (int j = 0; j < 6; j++) { f[2 * j] = magic_pair(b.q[j].x); f[2 * j + 1] = magic_pair(b.q[j].y); }
+    project3m<MU, SGN>(f, h);
+}
+// the stored integers of the upper (half = 0) or lower (half = 1) six complex numbers; the scale goes into the coefficient
+// the caller multiplies them with (raw_scale)
 MDWF_DEV void raw_half(const Raw &b, int half, c2 *v)
 {
-    const c2 s2 = dup(b.sc * (1.0f / MDWF_FIXED_MAX));
 #pragma unroll
-    for (int j = 0; j < 3; j++) { v[2 * j] = cvt_pair(b.q[3 * half + j].x, s2); v[2 * j + 1] = cvt_pair(b.q[3 * half + j].y, s2); }
+    for (int j = 0; j < 3; j++) { v[2 * j] = cvt_raw(b.q[3 * half + j].x); v[2 * j + 1] = cvt_raw(b.q[3 * half + j].y); }
 }
 MDWF_DEV void raw_full(const Raw &b, c2 *v)
 {
     raw_half(b, 0, v);
     raw_half(b, 1, v + 6);
 }
+MDWF_DEV float raw_scale(const Raw &b) { return b.sc * (1.0f / MDWF_FIXED_MAX); }
 MDWF_DEV void cp_async4(void *dst_smem, const void *src_gmem)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
@@ -327,9 +337,9 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
         }                                                                                               \
         Link U;                                                                                         \
         _Pragma("unroll") for (int k = 0; k < 9; k++) { U.re[k] = lw[cb_][k]; U.im[k] = lw[cb_][9 + k]; } \
-        c2 v[12], h[6], chi[6];                                                                         \
-        const float scw = raw_ints(nb[cb_], v);                                                         \
-        project3<MU, SGN>(v, h);                                                                        \
+        c2 h[6], chi[6];                                                                                \
+        const float scw = nb[cb_].sc * (1.0f / MDWF_FIXED_MAX);                                         \
+        project_magic<MU, SGN>(nb[cb_], h);                                                             \
         su3_mul3(U, h, chi);                                                                            \
         recon3<MU, SGN, true>(chi, (bs) * scw, acc);                                                    \
     } while (0)
@@ -386,12 +396,15 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 Raw ow[NB];
                 uint2 f_lo[3];                                                      // lower half of slice 0 as stored (wrap of s = L5-1)
                 float f_sc = 0.f;
-                c2 pu[6];
-                const c2 d2 = dup((float)a.own_d), o2 = dup((float)a.own_o), ow2 = dup((float)(-a.mf * a.own_o)), cf = dup(coef);
+                c2 pu[6];                                                           // upper half of slice s-1 (stored integers) and its scale
+                float pu_sc;
+                const float fd = (float)a.own_d, fo = (float)a.own_o, fow = (float)(-a.mf * a.own_o);
+                const c2 cf = dup(coef);
                 raw_ldg(ow[2], ob + (L5 - 1) * NV * 32, on + (L5 - 1) * 32);
                 raw_ldg(ow[0], ob, on);
                 raw_ldg(ow[1], ob + NV * 32, on + 32);
                 raw_half(ow[2], 0, pu);                                             // upper half of the last slice (wrap of s = 0)
+                pu_sc = raw_scale(ow[2]);
 #pragma unroll
                 for (int j = 0; j < 3; j++) f_lo[j] = ow[0].q[3 + j];
                 f_sc = ow[0].sc;
@@ -412,13 +425,15 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                                 for (int j = 0; j < 3; j++) nx.q[3 + j] = wrapl ? f_lo[j] : ow[(k + 1) % NB].q[3 + j];
                                 nx.sc = wrapl ? f_sc : ow[(k + 1) % NB].sc;
                                 raw_half(nx, 1, lo);
-                                const c2 fu = (s == 0) ? ow2 : o2, fl = wrapl ? ow2 : o2;
+                                const float csc = raw_scale(ow[k]);
+                                const c2 d2 = dup(fd * csc), fu = dup(((s == 0) ? fow : fo) * pu_sc), fl = dup((wrapl ? fow : fo) * raw_scale(nx));
 #pragma unroll
                                 for (int q = 0; q < 6; q++) {
                                     o[q] = fma2(d2, cur[q], mul2(fu, pu[q]));
                                     o[6 + q] = fma2(d2, cur[6 + q], mul2(fl, lo[q]));
                                     pu[q] = cur[q];
                                 }
+                                pu_sc = csc;
                             }
                             const unsigned hs = hit % HIST_SLOTS, hph = (hit / HIST_SLOTS) & 1;
                             mbar_wait(&hfull[w * HIST_SLOTS + hs], hph);
@@ -431,7 +446,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                             hit++;
 #pragma unroll
                             for (int q = 0; q < 12; q++) o[q] = fma2(cf, x[q], o[q]);
-                            nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                            nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                         }
                     }
                 }
@@ -485,7 +500,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                         zn[q] = zz;
                         o[DOFF / 2 + q] = fma2(qWd, zp[q], x[DOFF / 2 + q]);            // zp = z_{L5-1} of the direct half = its W
                     }
-                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 }
                 hit += L5;
             }
@@ -496,7 +511,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 static_assert(POST != 2 || OWN == 3, "POST = 2 comes with OWN = 3");
                 const unsigned h0 = hit;
                 const float cf = coef * (float)a.post_d, co = coef * (float)a.post_o, mw = (float)(-a.mf);
-                const c2 cd2 = dup(cf), od2 = dup((float)a.own_d);
+                const c2 cd2 = dup(cf);
                 constexpr int NB = 3;
                 Raw ow[NB];                                                         // slice j at index j % 3
                 raw_ldg(ow[0], ob, on);
@@ -512,15 +527,16 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
     } while (0)
                 // own-site term of output slice s: psi_s (rc), upper half of psi_{s+1} (ru), lower half of psi_{s-1} (rlo)
                 auto own_term = [&](int s, const Raw &rc, const Raw &ru, const Raw &rlo, c2 *o) {
-                    const c2 oou = dup((float)a.own_o * (s == L5 - 1 ? mw : 1.f)), ool = dup((float)a.own_o * (s == 0 ? mw : 1.f));
+                    const c2 oou = dup((float)a.own_o * (s == L5 - 1 ? mw : 1.f) * raw_scale(ru)), ool = dup((float)a.own_o * (s == 0 ? mw : 1.f) * raw_scale(rlo));
+                    const c2 odc = dup((float)a.own_d * raw_scale(rc));
                     c2 pc[12], pu[6], pl[6];
                     raw_full(rc, pc);
                     raw_half(ru, 0, pu);
                     raw_half(rlo, 1, pl);
 #pragma unroll
                     for (int q = 0; q < 6; q++) {
-                        o[q] = fma2(od2, pc[q], mul2(oou, pu[q]));
-                        o[6 + q] = fma2(od2, pc[6 + q], mul2(ool, pl[q]));
+                        o[q] = fma2(odc, pc[q], mul2(oou, pu[q]));
+                        o[6 + q] = fma2(odc, pc[6 + q], mul2(ool, pl[q]));
                     }
                 };
                 // hop part: x_s, the upper half of x_su and the lower half of x_sl from TMEM; then store
@@ -542,7 +558,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                     hist_load(tmem + HIST_COL0 + 24 * MDWF_HSLOT(s), x);
 #pragma unroll
                     for (int q = 0; q < 12; q++) o[q] = fma2(cd2, x[q], o[q]);
-                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 };
                 MDWF_HWAIT(0);
                 MDWF_HWAIT(1);
