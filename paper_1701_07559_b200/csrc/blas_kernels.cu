@@ -91,10 +91,10 @@ template <> struct CompT<PH, PH, PD> { using T = double; };
 // travel to the host ("unless kept on device")
 static thread_local const double *tl_coef = nullptr;
 void mdwf_blas_set_coef(const double *coef_dev) { tl_coef = coef_dev; }
-// S: [1] gamma, [2] ||q||^2, [3] ||r||^2, [4] gamma', [5..6] (alpha, 1) for r -= alpha q, [7..8] (alpha, beta) for the x / p update
+// S: [1] gamma, [2] ||q||^2, [3] ||r||^2, [4] gamma', [5..6] (alpha, 1) for r -= alpha q, [7..9] (alpha, beta, previous alpha) for the x / p update
 __global__ void cg_scalars_kernel(double *S, int mode)
 {
-    if (mode == 0) { const double al = S[1] / S[2]; S[5] = al; S[6] = 1.0; S[7] = al; }
+    if (mode == 0) { const double al = S[1] / S[2]; S[5] = al; S[6] = 1.0; S[9] = S[7]; S[7] = al; }   // S[9]: alpha of the iteration before
     else { S[8] = S[4] / S[1]; S[1] = S[4]; }
 }
 int mdwf_launch_cg_scalars(double *S, int mode, cudaStream_t st)
@@ -277,25 +277,37 @@ xpupdate_kernel(void *x, float *xn, double a, void *p, float *pn, double b, cons
 template <class PX, class PP>
 __global__ void __launch_bounds__(128)
 xpupdate_b_kernel(void *x, float *xn, double a, const void *p, const float *pn, double b, const void *g, const float *gn,
-                  void *pnew, float *pnewn, void *bp, float *bpn, float b5, float c5, float mf, int L5, long Vh, const double *coef)
+                  void *pnew, float *pnewn, void *bp, float *bpn, float b5, float c5, float mf, int L5, long Vh, const double *coef,
+                  int xmode)
 {
-    if (coef) { a *= coef[0]; b *= coef[1]; }
+    // xmode 1: x += a p.  The x update may run every other iteration (x is the widest vector of the update): xmode 0 leaves x
+    // alone, xmode 2 adds both pending terms, x += a_prev p_prev + a p, where p_prev is what the pnew buffer still holds (the
+    // double buffer of p) and is read slice by slice before the new p overwrites it.
+    double a_prev = 0.0;
+    if (coef) { a *= coef[0]; b *= coef[1]; a_prev = coef[2]; }
     // one thread walks the L5 slices of one 4D site, so every slice of p and g is loaded once: the new p of slice
     // s+1 is formed one step ahead, its lower spins feed B at s and its upper spins feed B at s+2
     using T = typename CompT<PX, PP, PP>::T;
     using RP = typename PP::R;
     const long cb = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= Vh) return;
-    const T ta = (T)a, tb = (T)b;
+    const T ta = (T)a, tb = (T)b, tap = (T)a_prev;
     RP cur[24], nxt[24], prev_up[12], first_low[12], vp[24], vg[24];
     auto new_p = [&](int s, RP *out, bool update_x) {
         load_spinor<PP>(p, pn, L5, s, cb, vp);
         load_spinor<PP>(g, gn, L5, s, cb, vg);
-        if (update_x) {
+        if (update_x && xmode != 0) {
             typename PX::R vx[24];
             load_spinor<PX>(x, xn, L5, s, cb, vx);
+            if (xmode == 2) {
+                RP vo[24];
+                load_spinor<PP>(pnew, pnewn, L5, s, cb, vo);
 #pragma unroll
-            for (int k = 0; k < 24; k++) vx[k] = (typename PX::R)((T)vx[k] + ta * (T)vp[k]);
+                for (int k = 0; k < 24; k++) vx[k] = (typename PX::R)((T)vx[k] + tap * (T)vo[k] + ta * (T)vp[k]);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 24; k++) vx[k] = (typename PX::R)((T)vx[k] + ta * (T)vp[k]);
+            }
             store_spinor<PX>(x, xn, L5, s, cb, vx);
         }
 #pragma unroll
@@ -330,11 +342,11 @@ xpupdate_b_kernel(void *x, float *xn, double a, const void *p, const float *pn, 
 }
 int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g,
                            const SpinorBuf &pnew, const SpinorBuf &bp, double b5, double c5, double mf, int L5, int Vh,
-                           cudaStream_t st)
+                           cudaStream_t st, int xmode)
 {
     const int nb = (Vh + 127) / 128;
 #define XB(PX) xpupdate_b_kernel<PX, PH><<<nb, 128, 0, st>>>(x.v, x.norm, a, p.v, p.norm, b, g.v, g.norm, pnew.v, \
-                                                                     pnew.norm, bp.v, bp.norm, (float)b5, (float)c5, (float)mf, L5, Vh, tl_coef)
+                                                                     pnew.norm, bp.v, bp.norm, (float)b5, (float)c5, (float)mf, L5, Vh, tl_coef, xmode)
     if (px == PREC_S) XB(PS);
     else if (px == PREC_H) XB(PH);
     else return (int)cudaErrorInvalidValue;

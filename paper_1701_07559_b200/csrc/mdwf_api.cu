@@ -729,9 +729,15 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
         double gam = 0;
         SpinorBuf pc = p, pn = p2;                                          // current / next direction vector (use_bp)
         // fused update; with use_bp it also writes B p_new and flips the double buffer of p
+        // With the double buffer of p (use_bp) the x update runs every other iteration: x_lo is the widest vector of the
+        // update (fp32 in the dsh ladder: 3.6 of its 7.5 GB), and the direction of the iteration before is still in the buffer
+        // the new p is about to overwrite.  x_pending = 1: alpha_k p_k has not been added yet (p_k = pn after the swap).
+        int x_pending = 0;
         auto cg_update = [&](double ax, double bx) -> int {
             if (use_bp) {
-                CUDA_OK(c, mdwf_launch_xpupdate_b(pxl, xlo, ax, pc, bx, g, pn, bpv, c->b5, c->c5, c->mf, c->L5, c->Vh, c->st));
+                const int xmode = (ax == 0.0) ? 0 : (x_pending ? 2 : 0);
+                CUDA_OK(c, mdwf_launch_xpupdate_b(pxl, xlo, ax, pc, bx, g, pn, bpv, c->b5, c->c5, c->mf, c->L5, c->Vh, c->st, xmode));
+                if (ax != 0.0) x_pending = !x_pending;
                 std::swap(pc, pn);
             } else {
                 CUDA_OK(c, mdwf_launch_xpupdate(pxl, xlo, ax, ps, pc, bx, g, c->L5, c->Vh, c->st));
@@ -766,6 +772,15 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
             TRY(v_axpby(c, ps, pc, 1.0, ps, g, 0.0, ps, nullptr, &dummy));  // p = g
             c->defer_slot = -1;
         }
+        // the pending term of the deferred x update: x_lo += alpha_k p_k (alpha_k = S[5], p_k = the buffer the update just left)
+        auto flush_x = [&]() -> int {
+            if (!x_pending) return MDWF_OK;
+            mdwf_blas_set_coef(S + 5);
+            const int rc = v_axpby(c, pxl, xlo, 1.0, ps, pn, 1.0, pxl, &xlo, nullptr);
+            mdwf_blas_set_coef(nullptr);
+            x_pending = 0;
+            return rc;
+        };
         while (k < maxiter && !converged) {
             c->defer_slot = 2;
             TRY(apply_Mpc(&dummy));                                         // q = Mpc p, ||q||^2
@@ -793,6 +808,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
                                 (c->max_update_interval > 0 && since_update >= c->max_update_interval);
             if (update) {
                 // reliable update: fold x_lo into x_hi, recompute the residual in fp64 and restart the sloppy residual from it
+                TRY(flush_x());
                 TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
                 TRY(v_zero(c, pxl, xlo));
                 TRY(opM(PDd, xhi, te, rhi, nullptr));
@@ -811,6 +827,7 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
             }
         }
         if (!converged) {   // fold what we have
+            TRY(flush_x());
             TRY(v_axpby(c, PDd, xhi, 1.0, pxl, xlo, 1.0, PDd, &xhi, nullptr));
         }
     }

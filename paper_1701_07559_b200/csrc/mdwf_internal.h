@@ -108,7 +108,7 @@ int mdwf_launch_xpupdate(Prec px, const SpinorBuf &x, double a, Prec pp, const S
 // 16-bit Krylov vectors: x += a p ; pnew = g + b p ; bp = (b5 + c5 Lambda) pnew   (p is not overwritten)
 int mdwf_launch_xpupdate_b(Prec px, const SpinorBuf &x, double a, const SpinorBuf &p, double b, const SpinorBuf &g,
                            const SpinorBuf &pnew, const SpinorBuf &bp, double b5, double c5, double mf, int L5, int Vh,
-                           cudaStream_t st);
+                           cudaStream_t st, int xmode = 1);   // xmode 0: x untouched, 1: x += a p, 2: x += coef[2] pnew_old + a p
 // device-resident CG scalars (blas_kernels.cu)
 void mdwf_blas_set_coef(const double *coef_dev);
 int mdwf_launch_cg_scalars(double *S, int mode, cudaStream_t st);
