@@ -118,6 +118,27 @@ int mdwf_blas_norm2(mdwf_ctx *ctx, const void *x_dev, long long n, int real_byte
 int mdwf_blas_redot(mdwf_ctx *ctx, const void *x_dev, const void *y_dev, long long n, int real_bytes, double *out);
 int mdwf_blas_axpy(mdwf_ctx *ctx, double a, const void *x_dev, void *y_dev, long long n, int real_bytes);
 
+/* ||x||^2 (S7, as mdwf_blas_norm2: same arithmetic, same fixed reduction order, bit-identical result) through an entry point
+ * that ALLOCATES NOTHING, for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it.  No context, no cudaMalloc / cudaFree / allocating library routine, no synchronisation, no host read-back:
+ * two kernels are queued on `stream` (a cudaStream_t, NULL = the default stream) and the result is written to out_dev.
+ *   x_dev    device pointer, n reals of real_bytes (8 or 4) bytes each; caller-owned, read only
+ *   out_dev  device pointer to ONE double; caller-owned, written when the queued kernels have run
+ * The per-block partial sums go to a scratch array that lives in the library image (a file-scope __device__ array of 4096 doubles
+ * = 32 KB; every GPU that loads the library holds it until the process exits).  Limits and sharing:
+ *   - n <= mdwf_noalloc_max_n() = 2^30 reals per call; beyond it the call returns MDWF_EARG and touches nothing;
+ *   - every call on a device shares that one array, which keeps the last call's contents (nothing in it needs clearing: a call
+ *     overwrites exactly the partials it reads back).  Calls that overlap on the GPU (different streams, or host threads whose
+ *     launches are not ordered) RACE on it and give wrong results: the caller serialises them.
+ * mdwf_noalloc_setup() takes the array's device address for the current device (cudaGetSymbolAddress; first use also loads the
+ * module): call it once per device outside any graph capture; mdwf_blas_norm2_noalloc does it itself on first use otherwise.
+ * Errors: MDWF_EARG (n < 0, n beyond the maximum, real_bytes, null pointer), MDWF_ECUDA; text in mdwf_noalloc_last_error()
+ * (per host thread). */
+int mdwf_blas_norm2_noalloc(const void *x_dev, long long n, int real_bytes, double *out_dev, void *stream);
+int mdwf_noalloc_setup(void);
+long long mdwf_noalloc_max_n(void);
+const char *mdwf_noalloc_last_error(void);
+
 /* 4D <-> 5D maps either side of the solve (Eq. (5), defines the quark field on the
  * walls and the midpoint field of the residual-mass ratio).  4D fields are eta[t][z][y][x][spin][colour] (V4 x 24 reals).
  * mdwf_wall_source: src(x,s) = delta_{s,0} P+ eta(x) + delta_{s,L5-1} P- eta(x) (lift = 0), or D_- applied to it (lift = 1;

@@ -16,7 +16,8 @@ OP_MPC, OP_MPCDAG, OP_MDAGM, OP_D, OP_DDAG, OP_MPC_SYM, OP_MPCDAG_SYM = 0, 1, 2,
 EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", "mdwf_load_gauge_host",
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
            "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
-           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project", "mdwf_gradient_flow", "mdwf_plaquette"]
+           "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project", "mdwf_gradient_flow", "mdwf_plaquette",
+           "mdwf_blas_norm2_noalloc", "mdwf_noalloc_setup", "mdwf_noalloc_max_n", "mdwf_noalloc_last_error"]
 
 _lib = None
 
@@ -46,6 +47,12 @@ def lib():
         L.mdwf_solve_host.argtypes = [P, P, P, D, I, ctypes.POINTER(I), ctypes.POINTER(D)]
         L.mdwf_blas_norm2.argtypes = [P, P, LL, I, ctypes.POINTER(D)]
         L.mdwf_blas_redot.argtypes = [P, P, P, LL, I, ctypes.POINTER(D)]
+        L.mdwf_blas_norm2_noalloc.argtypes = [P, LL, I, P, P]
+        L.mdwf_noalloc_setup.argtypes = []
+        L.mdwf_noalloc_max_n.argtypes = []
+        L.mdwf_noalloc_max_n.restype = LL
+        L.mdwf_noalloc_last_error.argtypes = []
+        L.mdwf_noalloc_last_error.restype = ctypes.c_char_p
         L.mdwf_blas_axpy.argtypes = [P, D, P, P, LL, I]
         L.mdwf_get_stat.argtypes = [P, ctypes.c_char_p, ctypes.POINTER(D)]
         L.mdwf_last_error.argtypes = [P]
@@ -77,6 +84,27 @@ def _check(h, rc, allow=()):
     if rc != MDWF_OK and rc not in allow:
         raise MdwfError(rc, lib().mdwf_last_error(h).decode())
     return rc
+
+
+def blas_norm2_noalloc(x, out, stream=None):
+    """||x||^2 of the device tensor x into the one-element fp64 device tensor `out`, through the entry point that allocates
+    nothing (include/mdwf.h); queued on `stream` (a raw cudaStream_t handle, default stream if None), not synchronised."""
+    n = x.numel() * (2 if x.is_complex() else 1)
+    rb = Mdwf._rb(x)
+    rc = lib().mdwf_blas_norm2_noalloc(x.data_ptr(), n, rb, out.data_ptr(), stream)
+    if rc != MDWF_OK:
+        raise MdwfError(rc, lib().mdwf_noalloc_last_error().decode())
+    return rc
+
+
+def noalloc_setup():
+    rc = lib().mdwf_noalloc_setup()
+    if rc != MDWF_OK:
+        raise MdwfError(rc, lib().mdwf_noalloc_last_error().decode())
+
+
+def noalloc_max_n():
+    return int(lib().mdwf_noalloc_max_n())
 
 
 def mdwf_destroy(h):
