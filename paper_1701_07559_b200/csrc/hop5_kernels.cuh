@@ -109,6 +109,13 @@ MDWF_DEV void tm_wait_ld24(float *a, float *b)
                    "+f"(b[8]), "+f"(b[9]), "+f"(b[10]), "+f"(b[11])
                  :);
 }
+MDWF_DEV void tm_wait_ld12(float *a)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+f"(a[4]), "+f"(a[5]), "+f"(a[6]), "+f"(a[7]), "+f"(a[8]), "+f"(a[9]),
+                   "+f"(a[10]), "+f"(a[11])
+                 :);
+}
 // 24 words of one slice slot <-> 12 complex pairs
 MDWF_DEV void hist_store(unsigned ta, const c2 *x)
 {
@@ -171,6 +178,10 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
     static_assert(PRE == 0, "v5: B-on-load not yet");
     constexpr int NV = P::NV;
     constexpr unsigned SLOT = SL::BYTES;
+    // history ring: POST = 2 gives up one slot for 36 parked columns (out_0 without its x_{L5-1} term, upper half of x_0)
+    constexpr int NS = (POST == 2) ? HIST_SLOTS - 1 : HIST_SLOTS;
+    constexpr int PARK0 = HIST_COL0 + 24 * (HIST_SLOTS - 1), PARK1 = PARK0 + 24;
+    static_assert(PARK1 + 12 <= 512, "tensor memory columns");
     extern __shared__ __align__(128) unsigned char smem5[];
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem5 + RING * SLOT);
     unsigned long long *full = bars, *empty = bars + RING;                          // ring: producer -> sweep, sweep -> producer
@@ -394,7 +405,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
                 MDWF_DIR5(3, true, true, 6, btp);
                 MDWF_DIR5(3, false, true, 7, btm);
                 // ---- raw hop result of the slice -> TMEM history slot, handed to the epilogue warp of the same lanes ----
-                const unsigned hs = hit % HIST_SLOTS, hph = (hit / HIST_SLOTS) & 1;
+                const unsigned hs = hit % NS, hph = (hit / NS) & 1;
                 mbar_wait(&hempty[warp * HIST_SLOTS + hs], hph ^ 1);
                 tm_fence_after();
                 hist_store(tmem + HIST_COL0 + 24 * hs, acc);
@@ -435,7 +446,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
 #pragma unroll
                         for (int q = 0; q < 6; q++) first_lo[q] = cur[6 + q];
                     }
-                    const unsigned hs = hit % HIST_SLOTS, hph = (hit / HIST_SLOTS) & 1;
+                    const unsigned hs = hit % NS, hph = (hit / NS) & 1;
                     mbar_wait(&hfull[w * HIST_SLOTS + hs], hph);
                     tm_fence_after();
                     c2 x[12], o[12];
@@ -478,7 +489,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
 #pragma unroll
                 for (int q = 0; q < 6; q++) { zp[q] = mk(0.f, 0.f); Wm[q] = mk(0.f, 0.f); }
                 for (int s = 0; s < L5; s++) {
-                    const unsigned hs = (h0 + s) % HIST_SLOTS, hph = ((h0 + s) / HIST_SLOTS) & 1;
+                    const unsigned hs = (h0 + s) % NS, hph = ((h0 + s) / NS) & 1;
                     mbar_wait(&hfull[w * HIST_SLOTS + hs], hph);
                     tm_fence_after();
                     c2 x[12];
@@ -502,7 +513,7 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
 #pragma unroll
                 for (int q = 0; q < 6; q++) zn[q] = mk(0.f, 0.f);
                 for (int s = L5 - 1; s >= 0; s--) {
-                    const unsigned hs = (h0 + s) % HIST_SLOTS;
+                    const unsigned hs = (h0 + s) % NS;
                     c2 x[12], o[12];
                     hist_load(tmem + HIST_COL0 + 24 * hs, x);
                     tm_fence_before();
@@ -523,8 +534,8 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
             if (POST == 2) {
                 // out_s = coef (post_d + post_o Lambda^dagger) x_s + (own_d + own_o Lambda^dagger) psi_s   (OWN = 3):
                 // upper spins take slice s+1, lower spins slice s-1, factor -m_f at the wrap.  Streaming: out_s is finished as
-                // soon as x_{s+1} has arrived (s = 1 .. L5-2), then s = L5-1 and s = 0, which need the other end of the fifth
-                // dimension; the history slots of x_0 and x_1 are kept until then.  The own slices sit in a rotating
+                // soon as x_{s+1} has arrived (s = 1 .. L5-2) and every history slot is freed as soon as the next output has used it;
+                // then s = L5-1 and s = 0, which need the other end of the fifth dimension.  The own slices sit in a rotating
                 // register window (s-1 .. s+2), each loaded from global memory once.
                 static_assert(POST != 2 || OWN == 3, "POST = 2 comes with OWN = 3");
                 const V *ob = reinterpret_cast<const V *>(a.own) + g * (long)(L5 * NV * 32) + lane;
@@ -536,8 +547,8 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
                 Ld<P>::template chunks<12>(ob, 1.f, ow[0]);
                 Ld<P>::template chunks<12>(ob + NV * 32, 1.f, ow[1]);
                 Ld<P>::template chunks<12>(ob + 2 * NV * 32, 1.f, ow[2]);
-#define MDWF_HSLOT(s_) ((h0 + (unsigned)(s_)) % HIST_SLOTS)
-#define MDWF_HWAIT(s_) mbar_wait(&hfull[w * HIST_SLOTS + MDWF_HSLOT(s_)], ((h0 + (unsigned)(s_)) / HIST_SLOTS) & 1)
+#define MDWF_HSLOT(s_) ((h0 + (unsigned)(s_)) % NS)
+#define MDWF_HWAIT(s_) mbar_wait(&hfull[w * HIST_SLOTS + MDWF_HSLOT(s_)], ((h0 + (unsigned)(s_)) / NS) & 1)
 #define MDWF_HFREE(s_)                                                                   \
     do {                                                                                 \
         tm_fence_before();                                                               \
@@ -564,25 +575,66 @@ __global__ void __launch_bounds__(384, 1) hop5_kernel(const HopArgs a)
                 };
                 MDWF_HWAIT(0);
                 MDWF_HWAIT(1);
+                tm_fence_after();
+                // So that slots 0 and 1 are not held until the two ends are done (the sweep of the next tile would wait for the
+                // whole tail of this one), what they contribute there is parked in 36 tensor-memory columns of this warp's own:
+                // out_0 without its x_{L5-1} term, and the upper half of x_0.
+                {
+                    c2 lastlo[6], o[12], x[12];
+                    Ld<P>::template chunks<6>(ob + (L5 - 1) * NV * 32 + 32 * (NV / 2), 1.f, lastlo);   // lower half of psi_{L5-1}
+                    float xu[12], pk[12];
+                    const unsigned tu = tmem + HIST_COL0 + 24 * MDWF_HSLOT(1);
+                    tm_ld8(tu, xu); tm_ld2(tu + 8, xu + 8); tm_ld2(tu + 10, xu + 10);
+                    hist_load(tmem + HIST_COL0 + 24 * MDWF_HSLOT(0), x);
+                    tm_wait_ld12(xu);
+                    const c2 cou = dup(co), oou = dup((float)a.own_o), ool = dup((float)a.own_o * mw);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) {
+                        o[q] = fma2(cd2, x[q], fma2(cou, mk(xu[2 * q], xu[2 * q + 1]), fma2(od2, ow[0][q], mul2(oou, ow[1][q]))));
+                        o[6 + q] = fma2(cd2, x[6 + q], fma2(od2, ow[0][6 + q], mul2(ool, lastlo[q])));
+                        pk[2 * q] = x[q].x; pk[2 * q + 1] = x[q].y;
+                    }
+                    hist_store(tmem + PARK0, o);
+                    tm_st8(tmem + PARK1, pk);
+                    tm_st2(tmem + PARK1 + 8, pk + 8);
+                    tm_st2(tmem + PARK1 + 10, pk + 10);
+                    tm_wait_st();
+                }
+                c2 up0[6];                                                          // upper half of psi_0 (own term of out_{L5-1}), read again late
 #pragma unroll
                 for (int s = 1; s <= L5 - 2; s++) {
                     if (s + 2 <= L5 - 1) Ld<P>::template chunks<12>(ob + (s + 2) * NV * 32, 1.f, ow[(s + 2) % NB]);
+                    if (s == L5 - 2) Ld<P>::template chunks<6>(ob, 1.f, up0);
                     MDWF_HWAIT(s + 1);
                     tm_fence_after();
                     finish(s, s + 1, s - 1, ow[s % NB], ow[(s + 1) % NB], ow[(s - 1) % NB]);
-                    if (s - 1 >= 2) MDWF_HFREE(s - 1);
+                    MDWF_HFREE(s - 1);
                 }
-                // the two ends: s = L5-1 (upper from slice 0) and s = 0 (lower from slice L5-1); psi_0, psi_1 are read again
-                c2 p0[12], p1[6];
-                Ld<P>::template chunks<12>(ob, 1.f, p0);
-                Ld<P>::template chunks<6>(ob + NV * 32, 1.f, p1);
-                finish(L5 - 1, 0, L5 - 2, ow[(L5 - 1) % NB], p0, ow[(L5 - 2) % NB]);
-                finish(0, 1, L5 - 1, p0, p1, ow[(L5 - 1) % NB]);
+                {   // the two ends: out_{L5-1} (upper from the parked x_0, lower from x_{L5-2}) and the rest of out_0
+                    const c2 *pc = ow[(L5 - 1) % NB], *pl = ow[(L5 - 2) % NB];
+                    c2 o[12], x[12];
+                    float xu[12], xl[12];
+                    const unsigned tl = tmem + HIST_COL0 + 24 * MDWF_HSLOT(L5 - 2) + 12;
+                    tm_ld8(tmem + PARK1, xu); tm_ld2(tmem + PARK1 + 8, xu + 8); tm_ld2(tmem + PARK1 + 10, xu + 10);
+                    tm_ld8(tl, xl); tm_ld2(tl + 8, xl + 8); tm_ld2(tl + 10, xl + 10);
+                    tm_wait_ld24(xu, xl);
+                    hist_load(tmem + HIST_COL0 + 24 * MDWF_HSLOT(L5 - 1), x);
+                    const c2 cou = dup(co * mw), col = dup(co), oou = dup((float)a.own_o * mw), ool = dup((float)a.own_o);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) {
+                        o[q] = fma2(cd2, x[q], fma2(cou, mk(xu[2 * q], xu[2 * q + 1]), fma2(od2, pc[q], mul2(oou, up0[q]))));
+                        o[6 + q] = fma2(cd2, x[6 + q], fma2(col, mk(xl[2 * q], xl[2 * q + 1]), fma2(od2, pc[6 + q], mul2(ool, pl[6 + q]))));
+                    }
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, L5 - 1, cb, o, a.partial != nullptr);
+                    hist_load(tmem + PARK0, o);
+                    const c2 colw = dup(co * mw);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) o[6 + q] = fma2(colw, x[6 + q], o[6 + q]);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, 0, cb, o, a.partial != nullptr);
+                }
                 tm_fence_before();
                 __syncwarp();
                 if (lane == 0) {
-                    mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(0)]);
-                    mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(1)]);
                     mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(L5 - 2)]);
                     mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(L5 - 1)]);
                 }

@@ -95,6 +95,10 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
     constexpr int NV = 6, RING = SL::RING;
     constexpr unsigned SLOT = SL::BYTES;
     constexpr unsigned ITEMS = 2 + L5;                                               // ring items per tile: 2 of links, L5 slices
+    // history ring: POST = 2 gives up one slot for 36 parked columns (partial out_0, upper half of x_0: see its epilogue)
+    constexpr int NS = (POST == 2) ? HIST_SLOTS - 1 : HIST_SLOTS;
+    constexpr int PARK0 = HIST_COL0 + 24 * (HIST_SLOTS - 1), PARK1 = PARK0 + 24;
+    static_assert(PARK1 + 12 <= 512, "tensor memory columns");
     extern __shared__ __align__(128) unsigned char smem6[];
     unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem6 + RING * SLOT);
     unsigned long long *full = bars, *empty = bars + RING;                          // ring: producers -> sweep, sweep -> producers
@@ -357,7 +361,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 MDWF_DIR6(3, true, 6, btp);
                 MDWF_DIR6(3, false, 7, btm);
                 // ---- raw hop result of the slice -> TMEM history slot, handed to the epilogue warp of the same lanes ----
-                const unsigned hit = h0 + s, hs = hit % HIST_SLOTS, hph = (hit / HIST_SLOTS) & 1;
+                const unsigned hit = h0 + s, hs = hit % NS, hph = (hit / NS) & 1;
                 mbar_wait(&hempty[w * HIST_SLOTS + hs], hph ^ 1);
                 tm_fence_after();
                 hist_store(tmem + HIST_COL0 + 24 * hs, acc);
@@ -435,7 +439,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                                 }
                                 pu_sc = csc;
                             }
-                            const unsigned hs = hit % HIST_SLOTS, hph = (hit / HIST_SLOTS) & 1;
+                            const unsigned hs = hit % NS, hph = (hit / NS) & 1;
                             mbar_wait(&hfull[w * HIST_SLOTS + hs], hph);
                             tm_fence_after();
                             c2 x[12];
@@ -462,7 +466,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 #pragma unroll
                 for (int q = 0; q < 6; q++) { zp[q] = mk(0.f, 0.f); Wm[q] = mk(0.f, 0.f); }
                 for (int s = 0; s < L5; s++) {
-                    const unsigned hs = (h0 + s) % HIST_SLOTS, hph = ((h0 + s) / HIST_SLOTS) & 1;
+                    const unsigned hs = (h0 + s) % NS, hph = ((h0 + s) / NS) & 1;
                     mbar_wait(&hfull[w * HIST_SLOTS + hs], hph);
                     tm_fence_after();
                     c2 x[12];
@@ -486,7 +490,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 #pragma unroll
                 for (int q = 0; q < 6; q++) zn[q] = mk(0.f, 0.f);
                 for (int s = L5 - 1; s >= 0; s--) {
-                    const unsigned hs = (h0 + s) % HIST_SLOTS;
+                    const unsigned hs = (h0 + s) % NS;
                     c2 x[12], o[12];
                     hist_load(tmem + HIST_COL0 + 24 * hs, x);
                     tm_fence_before();
@@ -505,9 +509,12 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 hit += L5;
             }
             if (POST == 2) {
-                // out_s = coef (post_d + post_o Lambda^dagger) x_s + (own_d + own_o Lambda^dagger) psi_s   (OWN = 3), streaming as
-                // in hop5_kernels.cuh: out_s once x_{s+1} has arrived (s = 1 .. L5-2), then the two ends.  The own slices sit as
-                // stored in a rotating window of three (s-1, s, s+1); the loop is rolled by the window length.
+                // out_s = coef (post_d + post_o Lambda^dagger) x_s + (own_d + own_o Lambda^dagger) psi_s   (OWN = 3), streaming:
+                // out_s once x_{s+1} has arrived (s = 1 .. L5-2), every history slot freed as soon as the next output has used
+                // it.  The two ends need the other end of the fifth dimension; so that slots 0 and 1 are not held until then
+                // (the sweep of the next tile would wait for the whole tail of this one), what they contribute is parked in
+                // 36 tensor-memory columns of this warp's own: out_0 without its x_{L5-1} term, and the upper half of x_0.
+                // The own slices sit as stored in a rotating window of three (s-1, s, s+1); the loop is rolled by the window.
                 static_assert(POST != 2 || OWN == 3, "POST = 2 comes with OWN = 3");
                 const unsigned h0 = hit;
                 const float cf = coef * (float)a.post_d, co = coef * (float)a.post_o, mw = (float)(-a.mf);
@@ -517,8 +524,8 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 raw_ldg(ow[0], ob, on);
                 raw_ldg(ow[1], ob + NV * 32, on + 32);
                 raw_ldg(ow[2], ob + 2 * NV * 32, on + 64);
-#define MDWF_HSLOT(s_) ((h0 + (unsigned)(s_)) % HIST_SLOTS)
-#define MDWF_HWAIT(s_) mbar_wait(&hfull[w * HIST_SLOTS + MDWF_HSLOT(s_)], ((h0 + (unsigned)(s_)) / HIST_SLOTS) & 1)
+#define MDWF_HSLOT(s_) ((h0 + (unsigned)(s_)) % NS)
+#define MDWF_HWAIT(s_) mbar_wait(&hfull[w * HIST_SLOTS + MDWF_HSLOT(s_)], ((h0 + (unsigned)(s_)) / NS) & 1)
 #define MDWF_HFREE(s_)                                                                   \
     do {                                                                                 \
         tm_fence_before();                                                               \
@@ -539,7 +546,8 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                         o[6 + q] = fma2(odc, pc[6 + q], mul2(ool, pl[q]));
                     }
                 };
-                // hop part: x_s, the upper half of x_su and the lower half of x_sl from TMEM; then store
+                // hop part: x_s, the upper half of x_su and the lower half of x_sl from TMEM; then store.  (Loading x_s and x_sl
+                // before the wait for x_{s+1} would save a tensor-memory latency per slice, but the extra live registers spill.)
                 auto finish = [&](int s, int su, int sl, c2 *o) {
                     const c2 cou = dup(co * (s == L5 - 1 ? mw : 1.f)), col = dup(co * (s == 0 ? mw : 1.f));
                     {
@@ -560,8 +568,39 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                     for (int q = 0; q < 12; q++) o[q] = fma2(cd2, x[q], o[q]);
                     nsum += (double)store3<P>(a.out, a.out_norm, L5, s, cb, o, a.partial != nullptr);
                 };
+                uint2 up0q[3];                                                      // upper half of psi_0 as stored: own term of out_{L5-1}
+#pragma unroll
+                for (int j = 0; j < 3; j++) up0q[j] = ow[0].q[j];
+                const float up0sc = ow[0].sc;
                 MDWF_HWAIT(0);
                 MDWF_HWAIT(1);
+                tm_fence_after();
+                {   // out_0 without col lo(x_{L5-1}): own term (lower half of psi_{L5-1} read here), x_0, upper half of x_1
+                    Raw lastlo;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) lastlo.q[3 + j] = __ldg(ob + (L5 - 1) * NV * 32 + 32 * (3 + j));
+                    lastlo.sc = __ldg(on + (L5 - 1) * 32);
+                    c2 o[12], x[12];
+                    own_term(0, ow[0], ow[1], lastlo, o);
+                    float xu[12];
+                    const unsigned tu = tmem + HIST_COL0 + 24 * MDWF_HSLOT(1);
+                    tm_ld8(tu, xu); tm_ld2(tu + 8, xu + 8); tm_ld2(tu + 10, xu + 10);
+                    hist_load(tmem + HIST_COL0 + 24 * MDWF_HSLOT(0), x);
+                    tm_wait_ld12(xu);
+                    const c2 cou = dup(co);
+                    float pk[12];
+#pragma unroll
+                    for (int q = 0; q < 6; q++) {
+                        o[q] = fma2(cd2, x[q], fma2(cou, mk(xu[2 * q], xu[2 * q + 1]), o[q]));
+                        o[6 + q] = fma2(cd2, x[6 + q], o[6 + q]);
+                        pk[2 * q] = x[q].x; pk[2 * q + 1] = x[q].y;
+                    }
+                    hist_store(tmem + PARK0, o);
+                    tm_st8(tmem + PARK1, pk);
+                    tm_st2(tmem + PARK1 + 8, pk + 8);
+                    tm_st2(tmem + PARK1 + 10, pk + 10);
+                    tm_wait_st();
+                }
 #pragma unroll 1
                 for (int s0 = 1; s0 <= L5 - 2; s0 += NB) {
 #pragma unroll
@@ -574,27 +613,39 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                             MDWF_HWAIT(s + 1);
                             tm_fence_after();
                             finish(s, s + 1, s - 1, o);
-                            if (s - 1 >= 2) MDWF_HFREE(s - 1);
+                            MDWF_HFREE(s - 1);
                         }
                     }
                 }
-                // the two ends: s = L5-1 (upper from slice 0) and s = 0 (lower from slice L5-1); psi_0, psi_1 are read again
-                // (keeping them in registers through the tile spills: measured slower)
-                {
-                    Raw p0, p1;
-                    raw_ldg(p0, ob, on);
-                    raw_ldg(p1, ob + NV * 32, on + 32);
-                    c2 o[12];
-                    own_term(L5 - 1, ow[(L5 - 1) % NB], p0, ow[(L5 - 2) % NB], o);
-                    finish(L5 - 1, 0, L5 - 2, o);
-                    own_term(0, p0, p1, ow[(L5 - 1) % NB], o);
-                    finish(0, 1, L5 - 1, o);
+                {   // the two ends: out_{L5-1} (upper from the parked x_0, lower from x_{L5-2}) and the rest of out_0
+                    Raw up0;
+#pragma unroll
+                    for (int j = 0; j < 3; j++) { up0.q[j] = up0q[j]; up0.q[3 + j] = up0q[j]; }
+                    up0.sc = up0sc;
+                    c2 o[12], x[12];
+                    own_term(L5 - 1, ow[(L5 - 1) % NB], up0, ow[(L5 - 2) % NB], o);
+                    float xu[12], xl[12];
+                    const unsigned tl = tmem + HIST_COL0 + 24 * MDWF_HSLOT(L5 - 2) + 12;
+                    tm_ld8(tmem + PARK1, xu); tm_ld2(tmem + PARK1 + 8, xu + 8); tm_ld2(tmem + PARK1 + 10, xu + 10);
+                    tm_ld8(tl, xl); tm_ld2(tl + 8, xl + 8); tm_ld2(tl + 10, xl + 10);
+                    tm_wait_ld24(xu, xl);
+                    hist_load(tmem + HIST_COL0 + 24 * MDWF_HSLOT(L5 - 1), x);
+                    const c2 cou = dup(co * mw), col = dup(co);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) {
+                        o[q] = fma2(cd2, x[q], fma2(cou, mk(xu[2 * q], xu[2 * q + 1]), o[q]));
+                        o[6 + q] = fma2(cd2, x[6 + q], fma2(col, mk(xl[2 * q], xl[2 * q + 1]), o[6 + q]));
+                    }
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, L5 - 1, cb, o, a.partial != nullptr);
+                    hist_load(tmem + PARK0, o);
+                    const c2 colw = dup(co * mw);
+#pragma unroll
+                    for (int q = 0; q < 6; q++) o[6 + q] = fma2(colw, x[6 + q], o[6 + q]);
+                    nsum += (double)store3<P>(a.out, a.out_norm, L5, 0, cb, o, a.partial != nullptr);
                 }
                 tm_fence_before();
                 __syncwarp();
                 if (lane == 0) {
-                    mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(0)]);
-                    mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(1)]);
                     mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(L5 - 2)]);
                     mbar_arrive(&hempty[w * HIST_SLOTS + MDWF_HSLOT(L5 - 1)]);
                 }
