@@ -237,11 +237,20 @@ def main():
         m.set_option("release_workspace", "1")
         for op, name in ((binding.OP_MPC, "Mpc"), (binding.OP_MPCDAG, "Mpcdag")):
             r = m.time_op(op, prec, reps=args.op_reps, warmup=3)
+            # The same pair the way the peak was measured (MEASURED_PEAKS.json: best of 10, a burst): 3 launches after 0.3 s
+            # of idle, best of 3 such bursts.  Back to back, these kernels pull the board to its 1000 W power cap within
+            # ~100 ms and the SM clock drops (fp32 tile sweep: 1965 -> ~1550 MHz); "ms" above is that
+            # sustained mean and the one every other number of this line is derived from.
+            burst = []
+            for _ in range(3):
+                time.sleep(0.3)
+                burst.append(m.time_op(op, prec, reps=3, warmup=1)["ms"])
             mpc["%s_%s" % (name, prec)] = {
                 "ms": r["ms"], "ms_k1": r["ms_k1"], "ms_k2": r["ms_k2"],
                 "tflops": F * h / (r["ms"] * 1e-3) / 1e12,
                 "GBs_model": b_site * h / (r["ms"] * 1e-3) / 1e9,
                 "frac_hbm": b_site * h / (r["ms"] * 1e-3) / 1e9 / hbm_peak,
+                "ms_burst": min(burst), "frac_hbm_burst": b_site * h / (min(burst) * 1e-3) / 1e9 / hbm_peak,
                 "bytes_per_site_model": b_site}
     m.set_option("release_workspace", "1")     # the timing vectors make room for the solver's (configs[4]: 157 GB in use)
     torch.cuda.empty_cache()

@@ -7,6 +7,7 @@ Few launches, so it is the command the ncu captures under profiles/ are taken wi
 """
 import argparse
 import json
+import time
 
 import torch
 
@@ -24,6 +25,9 @@ def main():
     ap.add_argument("--fma-rates", action="store_true", help="also print the measured FFMA / FFMA2 rates")
     ap.add_argument("--l2-rates", action="store_true", help="also print the measured L2 -> SM and DRAM streaming rates")
     ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value")
+    ap.add_argument("--repeat", type=int, default=1, help="time every (op, precision) this many times in a row")
+    ap.add_argument("--sleep", type=float, default=0.0, help="idle seconds before each timing (burst against sustained: the "
+                    "kernels run into the board's power cap when launched back to back)")
     args = ap.parse_args()
     build.build()
     cfg = inputs.CONFIGS[args.workload]
@@ -46,7 +50,8 @@ def main():
     for prec in args.prec.split(","):
         rb, extra = {"fp64": (8, 0), "fp32": (4, 0), "half": (2, 4)}[prec]
         b_site = 5 * (24 * rb + extra) + 2 * 8 * recon * rb / L5
-        for op in (int(o) for o in args.ops.split(",")):
+        for op in (int(o) for o in args.ops.split(",") for _ in range(args.repeat)):
+            time.sleep(args.sleep)
             r = m.time_op(op, prec, reps=args.reps, warmup=args.warmup)
             r.update(op=("Mpc", "Mpcdag")[op], prec=prec, workload=cfg["name"], reconstruct=recon,
                      tflops=F * h / (r["ms"] * 1e-3) / 1e12, GBs_model=b_site * h / (r["ms"] * 1e-3) / 1e9)
