@@ -289,9 +289,11 @@ static int launch_hop_inst(const HopArgs &a, cudaStream_t st)
     size_t smem = 0;
     if (POST != 0) smem = ((size_t)L5 * 24 * 32 + (POST == 1 ? 2 * L5 * L5 : 0)) * sizeof(R);
     auto k = hop_kernel<P, DAG, PRE, POST, OWN, L5T, S>;
-    if (smem > 48 * 1024) {
+    static size_t smem_set = 0;                            // once per instantiation (and again only for a larger L5), not per launch
+    if (smem > 48 * 1024 && smem > smem_set) {
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
+        smem_set = smem;
     }
     k<<<grid, block, smem, st>>>(a);
     return (int)cudaGetLastError();
