@@ -136,6 +136,39 @@ def test_solve_other_L5(name):
     m.close()
 
 
+@pytest.mark.parametrize("name", ["tile8", "tile16"])
+@pytest.mark.parametrize("prec", ["fp32", "half"])
+def test_tile_sweep_with_18_real_links(name, prec):
+    """the tile-sweep kernels (forced: these lattices are below the size where `auto` picks them) reading uncompressed links"""
+    from paper_1701_07559_b200 import binding
+    orc, m, b = setup(name, "18")
+    m.set_option("kernels", "v5")
+    m.set_option("apply_precision", prec)
+    bo_full = orc.parity_part(b, 1)
+    x = to_dev(orc.pack_parity(b, 1), prec)
+    for op, r in ((binding.OP_MPC, orc.Mpc(bo_full)), (binding.OP_MPCDAG, orc.Mpcdag(bo_full))):
+        got = m.apply(op, x).cpu().numpy().astype(np.complex128)
+        assert rel(got, orc.pack_parity(r, 1)) < TOL[prec], (name, prec, op)
+    m.close()
+
+
+@pytest.mark.parametrize("ladder", ["ds", "dsh", "dh"])
+@pytest.mark.parametrize("name", ["tile8", "tile16", "lx32"])
+def test_solve_on_the_tile_sweep_kernels(name, ladder):
+    """whole solves on the forced tile-sweep kernels: hop5 (ds), hop6 with the B p stream and the x update that runs every other
+    iteration (dsh, dh); the oracle recomputes the residual.  A small update interval makes reliable updates fall on odd and on
+    even iterations (pending x term flushed / nothing pending)."""
+    orc, m, b = setup(name, "12")
+    m.set_option("kernels", "v5")
+    m.set_option("ladder", ladder)
+    for interval in (0, 7):
+        m.set_option("max_update_interval", str(interval))
+        sol, iters, tr, rc = m.solve(torch.from_numpy(b).cuda(), tol=1e-10, maxiter=5000)
+        assert rc == 0, (name, ladder, interval)
+        assert orc.true_residual(b, sol.cpu().numpy()) <= 1e-10, (name, ladder, interval)
+    m.close()
+
+
 @pytest.mark.parametrize("name,ladder", [("cfg1", "dsh"), ("lx32", "dsh"), ("ragged", "ds")])
 def test_solve_is_bit_reproducible(name, ladder):
     """fixed-order reductions everywhere (BLAS-1, fused norms of the hop epilogues): two solves agree bit for bit"""
