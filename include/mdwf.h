@@ -88,6 +88,9 @@ int mdwf_destroy(mdwf_ctx *ctx);
  *   "sweep_mb"        v2, v3: L2 budget in MB of one block-sweep slab (default 16; negative: lexicographic sweep).
  *   "release_workspace"  (any value) free the library's pooled work vectors now; they are reallocated on demand.
  *   "max_update_interval"  force a reliable update at least every n iterations (default "0": only the delta rule).
+ *   "time_hops"       "1": mdwf_solve records CUDA events around the four hop kernels of every CG iteration (K1, K2, K1^dagger,
+ *                     K2^dagger in the sloppy precision of the ladder); their average duration inside the solve is then in
+ *                     mdwf_get_stat "hop_ms_k1" | "hop_ms_k2" | "hop_ms_k1dag" | "hop_ms_k2dag" (counts: "hop_n_..."). Default "0".
  *   "matpc"           "asym" (default; the operator Chroma uses) | "sym": Schur system mdwf_solve iterates on.
  *                     sym: Mpc_sym x_o = A^{-1} b'_o with Mpc_sym = 1 - (1/4) A^{-1} H_oe B A^{-1} H_eo B ("significant reduction of
  *                     the condition number"); same source preparation, reconstruction and returned residual.
@@ -168,7 +171,8 @@ int mdwf_half_decode(mdwf_ctx *ctx, const void *words_dev, const void *scales_de
 
 /* Per-context counters.  Keys: "launches" (kernels launched so far), "iterations", "reliable_updates",
  * "solve_seconds" (device time of the last solve, CUDA events), "true_residual", "op_applications"
- * (Mpc + Mpc^dagger applications in the last solve, all precisions), "sloppy_applications". */
+ * (Mpc + Mpc^dagger applications in the last solve, all precisions), "sloppy_applications", and with option "time_hops" the
+ * "hop_ms_*" / "hop_n_*" keys described there. */
 int mdwf_get_stat(const mdwf_ctx *ctx, const char *key, double *value);
 
 const char *mdwf_last_error(const mdwf_ctx *ctx);

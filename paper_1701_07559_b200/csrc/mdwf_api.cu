@@ -91,6 +91,13 @@ struct mdwf_ctx {
     // stats
     double launches = 0, iterations = 0, reliable_updates = 0, solve_seconds = 0, true_residual = 0;
     double op_applications = 0, sloppy_applications = 0;
+    // option "time_hops": CUDA events around the four hop kernels of a CG iteration (sloppy precision) inside mdwf_solve, so that
+    // a kernel's average launch duration IN the timed solve can be reported beside the one measured alone (bench.py roofline)
+    int time_hops = 0;
+    int hop_time_prec = -1;          // >= 0 while a solve is running: the precision whose hop launches are timed
+    std::vector<cudaEvent_t> hop_ev; // pairs (before, after)
+    std::vector<int> hop_ev_tag;     // one tag per pair: 0 K1, 1 K2, 2 K1^dagger, 3 K2^dagger
+    double hop_ms[4] = {0, 0, 0, 0}, hop_n[4] = {0, 0, 0, 0};
     std::string err;
 };
 
@@ -296,7 +303,28 @@ static int run_hop(mdwf_ctx *c, Prec p, int dag, int pre, int post, int own, Hop
     a.kver = c->kver;
     a.t5_l2mb = c->tile_l2_mb;
     if (post == 1 && p != PREC_D && a.kver >= 3) fill_recurrence(c, a, ainv_only ? 1.0 : c->b5, ainv_only ? 0.0 : c->c5);   // coef (B A^{-1}) or coef A^{-1}
+    int tag = -1;
+    if (c->time_hops && (int)p == c->hop_time_prec) {
+        if (!dag && post == 1 && own == 0) tag = 0;
+        else if (!dag && post == 0 && own == 2) tag = 1;
+        else if (dag && post == 1 && own == 0) tag = 2;
+        else if (dag && post == 2 && own == 3) tag = 3;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (tag >= 0) {
+        const size_t k = c->hop_ev_tag.size();
+        if (c->hop_ev.size() < 2 * (k + 1)) {
+            CUDA_OK(c, cudaEventCreate(&e0));
+            c->hop_ev.push_back(e0);
+            CUDA_OK(c, cudaEventCreate(&e1));
+            c->hop_ev.push_back(e1);
+        }
+        e0 = c->hop_ev[2 * k]; e1 = c->hop_ev[2 * k + 1];
+        c->hop_ev_tag.push_back(tag);
+        CUDA_OK(c, cudaEventRecord(e0, c->st));
+    }
     CUDA_OK(c, mdwf_launch_hop(p, dag, pre, post, own, a, c->st));
+    if (tag >= 0) CUDA_OK(c, cudaEventRecord(e1, c->st));
     c->launches += 1;
     return MDWF_OK;
 }
@@ -498,6 +526,7 @@ int mdwf_destroy(mdwf_ctx *c)
     if (c->result_dev) cudaFree(c->result_dev);
     if (c->hop_partial) cudaFree(c->hop_partial);
     if (c->result_host) cudaFreeHost(c->result_host);
+    for (cudaEvent_t e : c->hop_ev) cudaEventDestroy(e);
     delete c;
     return MDWF_OK;
 }
@@ -529,6 +558,8 @@ int mdwf_set_option(mdwf_ctx *c, const char *key, const char *value)
         const double d = atof(value);
         if (!(d > 0.0 && d < 1.0)) { c->err = "reliable_delta must be in (0,1)"; return MDWF_EARG; }
         c->delta = d;
+    } else if (k == "time_hops") {
+        c->time_hops = atoi(value) != 0;
     } else if (k == "max_update_interval") {
         c->max_update_interval = atoi(value);
     } else if (k == "kernels") {
@@ -865,12 +896,24 @@ int mdwf_solve(mdwf_ctx *c, const void *src_dev, void *sol_dev, double tol, int 
     CUDA_OK(c, cudaEventCreate(&e0));
     if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); c->err = "cudaEventCreate"; return MDWF_ECUDA; }
     if (cudaEventRecord(e0, c->st) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); c->err = "cudaEventRecord"; return MDWF_ECUDA; }
+    c->hop_ev_tag.clear();
+    if (c->time_hops) c->hop_time_prec = (c->ladder == 0) ? (int)PREC_D : (c->ladder == 1 ? (int)PREC_S : (int)PREC_H);
     const int rc = solve_device(c, src_dev, sol_dev, tol, maxiter, iters_out, true_res_out);
+    c->hop_time_prec = -1;
     cudaEventRecord(e1, c->st);
     cudaEventSynchronize(e1);
     float ms = 0.f;
     cudaEventElapsedTime(&ms, e0, e1);
     c->solve_seconds = ms * 1e-3;
+    for (int t = 0; t < 4; t++) { c->hop_ms[t] = 0; c->hop_n[t] = 0; }
+    for (size_t k = 0; k < c->hop_ev_tag.size(); k++) {
+        float hm = 0.f;
+        if (cudaEventElapsedTime(&hm, c->hop_ev[2 * k], c->hop_ev[2 * k + 1]) == cudaSuccess) {
+            c->hop_ms[c->hop_ev_tag[k]] += hm;
+            c->hop_n[c->hop_ev_tag[k]] += 1;
+        }
+    }
+    c->hop_ev_tag.clear();
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     return rc;
@@ -1038,6 +1081,13 @@ int mdwf_get_stat(const mdwf_ctx *c, const char *key, double *value)
     else if (k == "true_residual") *value = c->true_residual;
     else if (k == "op_applications") *value = c->op_applications;
     else if (k == "sloppy_applications") *value = c->sloppy_applications;
+    else if (k.rfind("hop_ms_", 0) == 0 || k.rfind("hop_n_", 0) == 0) {     // option time_hops: average ms / count of the last solve
+        const bool ms = k[4] == 'm';
+        const std::string t = k.substr(ms ? 7 : 6);
+        const int tag = t == "k1" ? 0 : (t == "k2" ? 1 : (t == "k1dag" ? 2 : (t == "k2dag" ? 3 : -1)));
+        if (tag < 0) return MDWF_EARG;
+        *value = ms ? (c->hop_n[tag] > 0 ? c->hop_ms[tag] / c->hop_n[tag] : 0.0) : c->hop_n[tag];
+    }
     else return MDWF_EARG;
     return MDWF_OK;
 }
