@@ -1,21 +1,23 @@
-// hop6_kernels.cuh -- the tile sweep of hop5_kernels.cuh for 16-bit storage (fp32 arithmetic), with TWO sweep sets.
+// hop6_kernels.cuh -- the tile sweep of hop5_kernels.cuh for 16-bit storage (fp32 arithmetic), with two or three sweep sets.
 // Same tile (2(z) x 2(t) 32-site groups), same ring / TMEM / epilogue structure; what differs:
 //
 //   * a ring item holds the 16 regions of a slice as stored (4 x 16-bit fixed point per 8-byte chunk: 1.5 KB per group)
 //     plus their per-site scales (16 x 128 B): 26 KB instead of 48 KB, so 8 items fit and two slices can be worked on at
 //     once with six more on their way;
-//   * two sets of four sweep warps: set 0 takes the even slices, set 1 the odd ones.  The 16-bit sweep is bound by
+//   * NSET = 2 or 3 sets of four sweep warps: slice s belongs to set s % NSET.  The 16-bit sweep is bound by
 //     instruction issue (the conversions and the scale ride on top of the fp32 arithmetic), not by the memory system,
 //     and one warp per scheduler cannot hide its own latencies: two warps per scheduler can;
 //   * the sweep prefetches a neighbour as the 6 raw words + scale (7 registers) and converts at the point of use; the
 //     stored integers stay unscaled, the scale of the neighbour goes into the reconstruction weight (hop3_kernels.cuh);
-//   * set 0 writes the links of the tile into tensor memory, set 1 reads them (same lanes): two mbarriers per group
+//   * set 0 writes the links of the tile into tensor memory, the other sets read them (same lanes): two mbarriers per group
 //     (lready / lfree) order the two;
 //   * the per-site scales (own regions, halos) and the y-halo rows come in through 16- and 4-byte LDGSTS copies of the
 //     three helper warps; the TMA producer moves the 12 whole groups of a slice as before;
 //   * the epilogue warps prefetch their own-site slices raw as well (13 registers a slice) and quantise in store3<PH>.
 //
-// 16 warps (512 threads, 128 registers): sweep 0-7, epilogue 8-11, TMA producer 12, helpers 13-15.
+// NSET = 2: 16 warps (512 threads, 128 registers): sweep 0-7, epilogue 8-11, TMA producer 12, helpers 13-15.
+// NSET = 3 (K1, K1^dagger at L5 = 12; not the default, see launch_hop6_l5): 20 warps (640 threads, 96 registers): sweep 0-11, epilogue 12-15, producer 16, helpers 17-19; a
+// sweep warp then holds one neighbour and one link at a time (no prefetch): its two neighbours on the scheduler hide the latency.
 #pragma once
 #include "hop5_kernels.cuh"
 
@@ -85,13 +87,14 @@ MDWF_DEV void cp_async4(void *dst_smem, const void *src_gmem)
 }
 
 // =====================================================================================================================
-template <int DAG, int POST, int OWN, int L5>
-__global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
+template <int DAG, int POST, int OWN, int L5, int NSET>
+__global__ void __launch_bounds__(128 * NSET + 256, 1) hop6_kernel(const HopArgs a)
 {
     using P = PH;
     using G = typename P::G;
     using SL = S6;
-    static_assert(L5 % 2 == 0, "two sweep sets: even / odd slices");
+    static_assert(L5 % NSET == 0, "NSET sweep sets: slice s belongs to set s % NSET");
+    constexpr int W_EPI = 4 * NSET, W_TMA = W_EPI + 4, W_HLP = W_TMA + 1;      // first warp of each role
     constexpr int NV = 6, RING = SL::RING;
     constexpr unsigned SLOT = SL::BYTES;
     constexpr unsigned ITEMS = 2 + L5;                                               // ring items per tile: 2 of links, L5 slices
@@ -115,7 +118,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
     if (threadIdx.x == 0) {
         for (int i = 0; i < RING; i++) { mbar_init(&full[i], 97); mbar_init(&empty[i], 4); }   // full: expect_tx arrival + one LDGSTS arrival per helper lane
         for (int i = 0; i < 4 * HIST_SLOTS; i++) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], 1); }
-        for (int i = 0; i < 4; i++) { mbar_init(&lready[i], 1); mbar_init(&lfree[i], 1); }
+        for (int i = 0; i < 4; i++) { mbar_init(&lready[i], 1); mbar_init(&lfree[i], NSET - 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
     const unsigned tmem = *tmem_base_s + ((unsigned)(32 * (warp & 3)) << 16);       // this warp's lanes
 
     const int ntiles = a.t5_ntiles;
-    if (warp == 12) {
+    if (warp == W_TMA) {
         // ================= TMA producer: link tiles and the 12 whole groups of every slice =================
         const unsigned char *gin = reinterpret_cast<const unsigned char *>(a.in);
         const unsigned char *ggauge = reinterpret_cast<const unsigned char *>(a.gauge);
@@ -166,9 +169,9 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 it++;
             }
         }
-    } else if (warp >= 13) {
+    } else if (warp >= W_HLP) {
         // ================= helpers (warps 13-15): y-halo rows, scales of the 12 groups, scales of the y-halo rows =================
-        const int hw = warp - 13;
+        const int hw = warp - W_HLP;
         const unsigned char *gin = reinterpret_cast<const unsigned char *>(a.in);
         long *ys = ysrc + 48 * hw;
         unsigned *yd = ydst + 48 * hw;
@@ -230,7 +233,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 it++;
             }
         }
-    } else if (warp < 8) {
+    } else if (warp < W_EPI) {
         // ================= sweep warps: set 0 = warps 0-3 (even slices, writes the links), set 1 = warps 4-7 (odd slices) =================
         const int set = warp >> 2, w = warp & 3;
         const int pa = w & 1, pb = w >> 1;                                          // z / t offset of this warp's group in the tile
@@ -298,14 +301,19 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 
             // ---- the sweep of this set's slices, software-pipelined over (slice, direction) as in hop5_kernels.cuh ----
             constexpr int lk[8] = {0, 4, 1, 5, 2, 6, 3, 7};
-            Raw nb[2];
-            float lw[2][18];
+            // PF: the neighbour and the link of the NEXT direction are prefetched (two buffers each: 50 registers).  With three
+            // sweep sets a warp has 96 registers and two other sweep warps on its scheduler to hide its latencies: no prefetch.
+            constexpr bool PF = NSET < 3;
+            Raw nb[PF ? 2 : 1];
+            float lw[PF ? 2 : 1][18];
             unsigned it = it0 + 2 + set, slot = it % RING;
-            mbar_wait(&full[slot], (it / RING) & 1);
             const unsigned char *sb = smem6 + slot * SLOT;
-            raw_lds(nb[0], sb, MDWF_OFF(lk[0]), MDWF_NOFF(lk[0]));
-            tm_ld16(tmem + LINK_STRIDE * lk[0], lw[0]);
-            tm_ld2(tmem + LINK_STRIDE * lk[0] + 16, lw[0] + 16);
+            if constexpr (PF) {
+                mbar_wait(&full[slot], (it / RING) & 1);
+                raw_lds(nb[0], sb, MDWF_OFF(lk[0]), MDWF_NOFF(lk[0]));
+                tm_ld16(tmem + LINK_STRIDE * lk[0], lw[0]);
+                tm_ld2(tmem + LINK_STRIDE * lk[0] + 16, lw[0] + 16);
+            }
             int pending = -1;                                                       // history slot whose hand-off is not finished yet
 #define MDWF_HANDOFF()                                                                                  \
     do {                                                                                                \
@@ -320,14 +328,23 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 #define MDWF_DIR6(MU, FWD, d, bs)                                                                       \
     do {                                                                                                \
         constexpr int SGN = ((FWD) ? 1 : -1) * (DAG ? -1 : 1);                                          \
-        constexpr int cb_ = (d) & 1, nb_ = cb_ ^ 1;                                                     \
-        if ((d) < 7) {                                                                                  \
+        constexpr int cb_ = PF ? ((d) & 1) : 0, nb_ = PF ? (cb_ ^ 1) : 0;                               \
+        if constexpr (!PF) {                                                                            \
+            if ((d) == 0) {                                                                             \
+                slot = it % RING;                                                                       \
+                mbar_wait(&full[slot], (it / RING) & 1);                                                \
+                sb = smem6 + slot * SLOT;                                                               \
+            }                                                                                           \
+            raw_lds(nb[0], sb, MDWF_OFF(lk[(d)]), MDWF_NOFF(lk[(d)]));                                  \
+            tm_ld16(tmem + LINK_STRIDE * lk[(d)], lw[0]);                                               \
+            tm_ld2(tmem + LINK_STRIDE * lk[(d)] + 16, lw[0] + 16);                                      \
+        } else if ((d) < 7) {                                                                           \
             raw_lds(nb[nb_], sb, MDWF_OFF(lk[((d) + 1) & 7]), MDWF_NOFF(lk[((d) + 1) & 7]));            \
         } else {                                                                                        \
             __syncwarp();                                                                               \
             if (lane == 0) mbar_arrive(&empty[slot]);           /* every load of this ring item has been issued */ \
-            it += 2;                                                                                    \
-            if (s + 2 < L5) {                                                                           \
+            it += NSET;                                                                                 \
+            if (s + NSET < L5) {                                                                        \
                 slot = it % RING;                                                                       \
                 mbar_wait(&full[slot], (it / RING) & 1);                                                \
                 sb = smem6 + slot * SLOT;                                                               \
@@ -335,7 +352,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
             }                                                                                           \
         }                                                                                               \
         tm_wait_ld18(lw[cb_]);                                                                          \
-        if ((d) < 7 || s + 2 < L5) {                                                                    \
+        if (PF && ((d) < 7 || s + NSET < L5)) {                                                         \
             tm_ld16(tmem + LINK_STRIDE * lk[((d) + 1) & 7], lw[nb_]);                                   \
             tm_ld2(tmem + LINK_STRIDE * lk[((d) + 1) & 7] + 16, lw[nb_] + 16);                          \
         }                                                                                               \
@@ -346,8 +363,13 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
         project_magic<MU, SGN>(nb[cb_], h);                                                             \
         su3_mul3(U, h, chi);                                                                            \
         recon3<MU, SGN, true>(chi, (bs) * scw, acc);                                                    \
+        if (!PF && (d) == 7) {                                                                          \
+            __syncwarp();                                                                               \
+            if (lane == 0) mbar_arrive(&empty[slot]);           /* this ring item has been read */     \
+            it += NSET;                                                                                 \
+        }                                                                                               \
     } while (0)
-            for (int s = set; s < L5; s += 2) {
+            for (int s = set; s < L5; s += NSET) {
                 c2 acc[12];
 #pragma unroll
                 for (int q = 0; q < 12; q++) acc[q] = mk(0.f, 0.f);
@@ -368,7 +390,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
                 pending = (int)hs;
             }
             MDWF_HANDOFF();
-            if (set == 1) {                                                         // every link load of this tile has completed
+            if (set != 0) {                                                         // every link load of this tile has completed
                 tm_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&lfree[w]);
@@ -378,9 +400,9 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 #undef MDWF_OFF
 #undef MDWF_NOFF
         }
-    } else if (warp < 12) {
+    } else if (warp < W_TMA) {
         // ================= epilogue warps: fifth-dimension POST, own-site term, quantise + store, fused norm =================
-        const int w = warp - 8;
+        const int w = warp - W_EPI;
         const int pa = w & 1, pb = w >> 1;
         unsigned hit = 0;
         const float coef = (float)a.coef_hop;
@@ -667,7 +689,7 @@ __global__ void __launch_bounds__(512, 1) hop6_kernel(const HopArgs a)
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------------------
-template <int DAG, int POST, int OWN, int L5>
+template <int DAG, int POST, int OWN, int L5, int NSET>
 static int launch_hop6_inst(const HopArgs &a, cudaStream_t st)
 {
     static int sms = 0;
@@ -676,19 +698,26 @@ static int launch_hop6_inst(const HopArgs &a, cudaStream_t st)
         int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        cudaError_t e = cudaFuncSetAttribute(hop6_kernel<DAG, POST, OWN, L5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(hop6_kernel<DAG, POST, OWN, L5, NSET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) { sms = 0; return (int)e; }
     }
     const int grid = a.t5_ntiles < sms ? a.t5_ntiles : sms;
-    hop6_kernel<DAG, POST, OWN, L5><<<grid, 512, smem, st>>>(a);
+    hop6_kernel<DAG, POST, OWN, L5, NSET><<<grid, 128 * NSET + 256, smem, st>>>(a);
     return (int)cudaGetLastError();
 }
 template <int DAG, int POST, int OWN>
 static int launch_hop6_l5(const HopArgs &a, cudaStream_t st)
 {
-    if (a.L5 == 12) return launch_hop6_inst<DAG, POST, OWN, 12>(a, st);
+    // Three sweep sets (96 registers, no one-direction prefetch; build with -DMDWF_HOP6_NSET3) make K1 / K1^dagger faster when they
+    // are timed alone, 1.13 -> 1.09 ms, but the timed solve runs against the board's power cap and got SLOWER with them (3.06 ->
+    // 3.11 s, median SM clock 1905 -> 1830 MHz): two sets are the default.  The epilogues of K2 / K2^dagger (own-slice window) spill
+    // at 96 registers (1.23 -> 1.92 ms).
+#ifdef MDWF_HOP6_NSET3
+    if (a.L5 == 12) return launch_hop6_inst<DAG, POST, OWN, 12, POST == 1 ? 3 : 2>(a, st);
+#endif
+    if (a.L5 == 12) return launch_hop6_inst<DAG, POST, OWN, 12, 2>(a, st);
 #ifndef MDWF_DEV_FAST
-    if (a.L5 == 8) return launch_hop6_inst<DAG, POST, OWN, 8>(a, st);
+    if (a.L5 == 8) return launch_hop6_inst<DAG, POST, OWN, 8, 2>(a, st);
 #endif
     return -1;
 }
