@@ -104,6 +104,14 @@ int mdwf_load_gauge_host(mdwf_ctx *ctx, const void *U_host, int real_bytes);
 /* out = op(in).  ops 0-2, 5, 6: parity spinors (odd sites); ops 3-4: full 5D spinors.  in_dev != out_dev. */
 int mdwf_apply(mdwf_ctx *ctx, int op, const void *in_dev, void *out_dev, int real_bytes);
 
+/* The same operators on a BATCH of right-hand sides (a propagator is 12 spin-colour columns
+ * per source).  in_dev / out_dev hold nrhs parity vectors of mdwf_apply's layout back to back; op is MDWF_OP_MPC or
+ * MDWF_OP_MPCDAG; the arithmetic is fp32 on fp32 or 16-bit storage ("apply_precision" "fp32" (default here) | "half").  One kernel
+ * launch handles the whole batch: a thread block stages the link tile of its 32 sites once (and completes 12-real links once)
+ * for all nrhs vectors.  Results are bit-identical to nrhs calls of mdwf_apply in the same precision with "kernels" "v3".
+ * Errors: MDWF_EARG for other ops, nrhs outside 1..64, fp64, L5 outside {8, 12, 16} or |beta/alpha| >= 0.98. */
+int mdwf_apply_batch(mdwf_ctx *ctx, int op, int nrhs, const void *in_dev, void *out_dev, int real_bytes);
+
 /* Solve D x = src on the full 5D lattice (fp64 buffers): Schur preparation b' = b_o - D_oe A^{-1} b_e,
  * CG on Mpc^dagger Mpc (CGLS recurrences) with the configured precision ladder and reliable updates,
  * reconstruction x_e = A^{-1}(b_e - D_eo x_o).  tol is the target for ||src - D x|| / ||src||.

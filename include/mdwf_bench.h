@@ -31,6 +31,11 @@ int mdwf_fma_rates(mdwf_ctx *ctx, double *tfma2);
  * from DRAM.  These are the ceilings the hop kernels' L2 traffic is judged against (profiles/r02_l2_sm_ceiling.md). */
 int mdwf_l2_rates(mdwf_ctx *ctx, double *out4);
 
+/* The batched operator of mdwf_apply_batch on nrhs right-hand sides held in library buffers, timed with
+ * CUDA events: out2[0] = ms per batched application (K1 + K2, two launches for the whole batch), out2[1] = kernels launched.
+ * precision "fp32" | "half"; op MDWF_OP_MPC or MDWF_OP_MPCDAG; 1 <= nrhs <= 64. */
+int mdwf_time_op_batch(mdwf_ctx *ctx, int op, const char *precision, int nrhs, int reps, int warmup, double *out2);
+
 #ifdef __cplusplus
 }
 #endif

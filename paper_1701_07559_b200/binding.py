@@ -17,7 +17,7 @@ EXPORTS = ["mdwf_create", "mdwf_destroy", "mdwf_set_option", "mdwf_load_gauge", 
            "mdwf_apply", "mdwf_solve", "mdwf_solve_host", "mdwf_blas_norm2", "mdwf_blas_redot", "mdwf_blas_axpy",
            "mdwf_get_stat", "mdwf_last_error", "mdwf_flops_per_site", "mdwf_time_op", "mdwf_fma_rates",
            "mdwf_half_encode", "mdwf_half_decode", "mdwf_l2_rates", "mdwf_wall_source", "mdwf_wall_project", "mdwf_gradient_flow", "mdwf_plaquette",
-           "mdwf_blas_norm2_noalloc", "mdwf_noalloc_setup", "mdwf_noalloc_max_n", "mdwf_noalloc_last_error"]
+           "mdwf_apply_batch", "mdwf_time_op_batch", "mdwf_blas_norm2_noalloc", "mdwf_noalloc_setup", "mdwf_noalloc_max_n", "mdwf_noalloc_last_error"]
 
 _lib = None
 
@@ -48,6 +48,8 @@ def lib():
         L.mdwf_blas_norm2.argtypes = [P, P, LL, I, ctypes.POINTER(D)]
         L.mdwf_blas_redot.argtypes = [P, P, P, LL, I, ctypes.POINTER(D)]
         L.mdwf_blas_norm2_noalloc.argtypes = [P, LL, I, P, P]
+        L.mdwf_apply_batch.argtypes = [P, I, I, P, P, I]
+        L.mdwf_time_op_batch.argtypes = [P, I, ctypes.c_char_p, I, I, I, ctypes.POINTER(D)]
         L.mdwf_noalloc_setup.argtypes = []
         L.mdwf_noalloc_max_n.argtypes = []
         L.mdwf_noalloc_max_n.restype = LL
@@ -266,6 +268,19 @@ class Mdwf:
         out = torch.empty(words.shape[0], words.shape[1], 4, 3, dtype=dtype, device=words.device)
         _check(self.h, lib().mdwf_half_decode(self.h, words.data_ptr(), scales.data_ptr(), out.data_ptr(), self._rb(out)))
         return out
+
+    def apply_batch(self, op, x):
+        """x: (nrhs, Vh, L5, 4, 3) complex device tensor of parity vectors; returns Mpc / Mpc^dagger of each (NEXT-2)"""
+        import torch
+        assert x.is_contiguous() and x.is_cuda
+        out = torch.empty_like(x)
+        _check(self.h, lib().mdwf_apply_batch(self.h, op, x.shape[0], x.data_ptr(), out.data_ptr(), self._rb(x)))
+        return out
+
+    def time_op_batch(self, op, prec, nrhs, reps=10, warmup=3):
+        o = (ctypes.c_double * 2)()
+        _check(self.h, lib().mdwf_time_op_batch(self.h, op, prec.encode(), nrhs, reps, warmup, o))
+        return {"ms": o[0], "launches": o[1]}
 
     def norm2(self, x):
         v = ctypes.c_double(0.0)

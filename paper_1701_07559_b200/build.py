@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmdwf_b200.so")
 OBJDIR = os.path.join(HERE, "build")
 STAMP = os.path.join(HERE, "libmdwf_b200.stamp.json")
-SOURCES = ["mdwf_api.cu", "hop_d.cu", "hop_s.cu", "hop_h.cu", "hop3_s.cu", "hop3_h.cu", "hop5_s.cu", "hop6_h.cu", "blas_kernels.cu",
+SOURCES = ["mdwf_api.cu", "hop_d.cu", "hop_s.cu", "hop_h.cu", "hop3_s.cu", "hop3_h.cu", "hop3b_s.cu", "hop3b_h.cu", "hop5_s.cu", "hop6_h.cu", "blas_kernels.cu",
            "layout_kernels.cu", "flow_kernels.cu", "s5_kernels.cu", "peak_kernels.cu", "sdense_mma.cu", "noalloc_kernels.cu"]
 FLAGS = os.environ.get("MDWF_NVCC_EXTRA", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
                                                            "-std=c++17", "-Xcompiler", "-fPIC"]

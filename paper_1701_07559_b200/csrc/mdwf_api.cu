@@ -47,6 +47,14 @@ int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &
     default: return mdwf_launch_hop_H(dag, pre, post, own, a, st);
     }
 }
+int mdwf_launch_hop3_batch_S(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop3_batch_H(int, int, int, int, const HopArgs &, cudaStream_t);
+int mdwf_launch_hop_batch(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st)
+{
+    if (p == PREC_S) return mdwf_launch_hop3_batch_S(dag, pre, post, own, a, st);
+    if (p == PREC_H) return mdwf_launch_hop3_batch_H(dag, pre, post, own, a, st);
+    return -1;                               // fp64: no batched kernel (hop_kernels.cuh keeps no link tile)
+}
 int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, const void *dense,
                        cudaStream_t st)
 {
@@ -80,6 +88,7 @@ struct mdwf_ctx {
                              // 4 = the same with the t+- neighbour groups staged by TMA too, 2 = hop_kernels.cuh
     int tile_l2_mb = 0;      // v5: L2 budget (MB) of the working set of a z-chunk of tiles; 0 = default 48
     int sweep_mb = 0;        // L2 budget (MB) of one sweep slab; 0 = default 16, < 0 = lexicographic sweep
+    int sweep_rhs = 1;       // right-hand sides a block walks through per slab site (batched kernels): the slab holds that many vectors
     bool gauge_loaded = false;
     void *gauge[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
     void *dense[2][DENSE_KINDS] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};   // [0] double, [1] float
@@ -264,10 +273,11 @@ static HopArgs base_args(const mdwf_ctx *c, Prec p, int parity_out, const Spinor
     {
         const long plane = (long)(c->L[0] / 2) * c->L[1];
         const long rb = (p == PREC_D) ? 8 : (p == PREC_S ? 4 : 2);
-        const long budget = c->sweep_mb > 0 ? (long)c->sweep_mb << 20 : (16L << 20);
+        // (batched kernels: the slab holds sweep_rhs vectors per stream and gets half of the 126 MB L2)
+        const long budget = c->sweep_mb > 0 ? (long)c->sweep_mb << 20 : ((c->sweep_rhs > 1 ? 64L : 16L) << 20);
         int zc = 0;
         for (int d = 1; d <= c->L[2]; d++)
-            if (c->L[2] % d == 0 && (d * plane) % 32 == 0 && d * plane * 3 * c->L5 * 24 * rb <= budget) zc = d;
+            if (c->L[2] % d == 0 && (d * plane) % 32 == 0 && d * plane * 3 * c->L5 * 24 * rb * c->sweep_rhs <= budget) zc = d;
         if (c->sweep_mb < 0 || zc == c->L[2] || zc < 2) zc = 0;
         a.sweep_nb = zc ? (int)(zc * plane / 32) : 0;
         a.sweep_chunk = (int)(zc * plane);
@@ -636,6 +646,91 @@ int mdwf_load_gauge_host(mdwf_ctx *c, const void *U_host, int real_bytes)
     else rc = mdwf_load_gauge(c, tmp, real_bytes);
     cudaFree(tmp);
     return rc;
+}
+
+// ---- NEXT-2: Mpc / Mpc^dagger on a batch of right-hand sides (hop3b_kernels.cuh) -----------------------------------------
+// A batch is one spinor array over nrhs * Vp sites (Vp = Vh rounded up to 32): right-hand side r is the single-vector layout at
+// byte offset r * mdwf_spinor_bytes.
+static int get_spinor_batch(mdwf_ctx *c, const std::string &name, Prec p, int nrhs, SpinorBuf *out)
+{
+    const std::string key = name + ".x" + std::to_string(nrhs) + (p == PREC_D ? ".d" : p == PREC_S ? ".s" : ".h");
+    auto it = c->pool.find(key);
+    if (it != c->pool.end()) { *out = it->second; return MDWF_OK; }
+    SpinorBuf b;
+    CUDA_OK(c, cudaMalloc(&b.v, (size_t)nrhs * mdwf_spinor_bytes(p, c->L5, c->Vh)));
+    if (p == PREC_H) CUDA_OK(c, cudaMalloc((void **)&b.norm, sizeof(float) * (size_t)nrhs * c->L5 * ((c->Vh + 31) / 32 * 32)));
+    c->pool[key] = b;
+    *out = b;
+    return MDWF_OK;
+}
+static SpinorBuf batch_view(const mdwf_ctx *c, Prec p, const SpinorBuf &b, int r)
+{
+    SpinorBuf v = b;
+    v.v = (char *)b.v + (size_t)r * mdwf_spinor_bytes(p, c->L5, c->Vh);
+    if (b.norm) v.norm = b.norm + (size_t)r * c->L5 * ((c->Vh + 31) / 32 * 32);
+    return v;
+}
+static int run_hop_batch(mdwf_ctx *c, Prec p, int nrhs, int dag, int pre, int post, int own, HopArgs a)
+{
+    a.kver = 3;
+    a.nrhs = nrhs;
+    a.batch_sites = (c->Vh + 31) / 32 * 32;
+    if (post == 1) fill_recurrence(c, a, c->b5, c->c5);
+    const int rc = mdwf_launch_hop_batch(p, dag, pre, post, own, a, c->st);
+    if (rc == -1) { c->err = "batched kernels: fp32 / 16-bit storage, L5 in {8, 12, 16}, |beta/alpha| < 0.98 only"; return MDWF_EARG; }
+    CUDA_OK(c, rc);
+    c->launches += 1;
+    return MDWF_OK;
+}
+struct SweepRhs {            // base_args sizes the sweep slab for nrhs vectors while one of these is alive
+    mdwf_ctx *c;
+    SweepRhs(mdwf_ctx *c_, int nrhs) : c(c_) { c->sweep_rhs = nrhs; }
+    ~SweepRhs() { c->sweep_rhs = 1; }
+};
+static int op_Mpc_batch(mdwf_ctx *c, Prec p, int nrhs, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    SweepRhs guard(c, nrhs);
+    HopArgs k1 = base_args(c, p, 0, in, nullptr, tmp);        // K1: t_e = (B A^{-1}) H_eo (B in_o), every right-hand side
+    k1.coef_hop = c->b5; k1.pre_d = c->b5; k1.pre_o = c->c5;
+    TRY(run_hop_batch(c, p, nrhs, 0, 1, 1, 0, k1));
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2: out_o = A in_o - (1/4) H_oe t_e
+    k2.coef_hop = -0.25; k2.own_d = c->alpha; k2.own_o = c->beta;
+    return run_hop_batch(c, p, nrhs, 0, 0, 0, 2, k2);
+}
+static int op_Mpcdag_batch(mdwf_ctx *c, Prec p, int nrhs, const SpinorBuf &in, const SpinorBuf &tmp, const SpinorBuf &out)
+{
+    SweepRhs guard(c, nrhs);
+    HopArgs k1 = base_args(c, p, 0, in, nullptr, tmp);        // K1+: u_e = (A^{-+} B^+) H'_eo in_o
+    k1.coef_hop = 1.0;
+    TRY(run_hop_batch(c, p, nrhs, 1, 0, 1, 0, k1));
+    HopArgs k2 = base_args(c, p, 1, tmp, &in, out);           // K2+: out_o = A^+ in_o - (1/4) B^+ H'_oe u_e
+    k2.coef_hop = -0.25; k2.post_d = c->b5; k2.post_o = c->c5; k2.own_d = c->alpha; k2.own_o = c->beta;
+    return run_hop_batch(c, p, nrhs, 1, 0, 2, 3, k2);
+}
+int mdwf_apply_batch(mdwf_ctx *c, int op, int nrhs, const void *in_dev, void *out_dev, int real_bytes)
+{
+    TRY(check_ready(c));
+    if (!in_dev || !out_dev || in_dev == out_dev || (real_bytes != 8 && real_bytes != 4) || nrhs < 1 || nrhs > 64 ||
+        (op != MDWF_OP_MPC && op != MDWF_OP_MPCDAG)) {
+        c->err = "mdwf_apply_batch: bad argument (op must be Mpc or Mpc^dagger, 1 <= nrhs <= 64)";
+        return MDWF_EARG;
+    }
+    const Prec p = c->apply_prec >= 0 ? (Prec)c->apply_prec : PREC_S;
+    if (p == PREC_D) { c->err = "mdwf_apply_batch: fp32 or 16-bit apply_precision only"; return MDWF_EARG; }
+    SpinorBuf a, b, t;
+    TRY(get_spinor_batch(c, "bt.a", p, nrhs, &a));
+    TRY(get_spinor_batch(c, "bt.b", p, nrhs, &b));
+    TRY(get_spinor_batch(c, "bt.t", p, nrhs, &t));
+    const size_t vec = (size_t)c->Vh * c->L5 * 24 * real_bytes;              // one parity vector of the caller
+    for (int r = 0; r < nrhs; r++)
+        CUDA_OK(c, mdwf_launch_parity_in(p, (const char *)in_dev + r * vec, real_bytes, batch_view(c, p, a, r), c->L5, c->Vh, c->st));
+    if (op == MDWF_OP_MPC) TRY(op_Mpc_batch(c, p, nrhs, a, t, b));
+    else TRY(op_Mpcdag_batch(c, p, nrhs, a, t, b));
+    for (int r = 0; r < nrhs; r++)
+        CUDA_OK(c, mdwf_launch_parity_out(p, batch_view(c, p, b, r), (char *)out_dev + r * vec, real_bytes, c->L5, c->Vh, c->st));
+    c->launches += 2 * nrhs;
+    CUDA_OK(c, cudaStreamSynchronize(c->st));
+    return MDWF_OK;
 }
 
 int mdwf_apply(mdwf_ctx *c, int op, const void *in_dev, void *out_dev, int real_bytes)

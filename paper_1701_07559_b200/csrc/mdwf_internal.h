@@ -76,6 +76,9 @@ struct HopArgs {
     float r_bz, r_cz;        // coef_hop b5/alpha, coef_hop c5/alpha
     float r_qC[4];           // coef_hop (b5 p_j + c5 p_{j-1})/alpha, p_j = (-kappa)^{j+1}, p_{-1} = 1
     float r_qW[32];          // coef_hop * wall term of slice s (effective index): -g m_f (b5 (-kappa)^{s+1} + c5 (-kappa)^s)
+    // batched kernels (hop3b_kernels.cuh, NEXT-2): in / own / out hold nrhs vectors, right-hand side r at site indices [r batch_sites, ...)
+    int nrhs;
+    int batch_sites;         // Vh rounded up to a multiple of 32
     // v5 tile-sweep kernels (hop5_kernels.cuh): tile geometry, filled by the launcher
     int t5_NY, t5_nzq, t5_NT, t5_ntiles;   // 32-site groups along y, z-pairs per chunk, t-pairs, tiles
     int t5_l2mb;                           // L2 budget (MB) of a z-chunk's working set; 0 = default 48
@@ -86,6 +89,8 @@ struct HopArgs {
 // s-matrix, 2 bidiagonal Lambda^dagger form.  own: 0 none, 1 + psi_own, 2 + (d + o Lambda) psi_own,
 // 3 + (d + o Lambda^dagger) psi_own.  Returns cudaError_t as int.
 int mdwf_launch_hop(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st);
+// the same on a batch of a.nrhs right-hand sides (fp32 arithmetic only; Mpc / Mpc^dagger kernels); -1 = not covered
+int mdwf_launch_hop_batch(Prec p, int dag, int pre, int post, int own, const HopArgs &a, cudaStream_t st);
 
 // site-local dense s-matrix: out = M in (M = R[2][L5][L5] on device, in the precision's compute type)
 int mdwf_launch_sdense(Prec p, int L5, int Vh, const SpinorBuf &in, const SpinorBuf &out, const void *dense,

@@ -81,3 +81,42 @@ def test_gradient_flow_parity(action, L):
     assert np.max(np.abs(got - ref)) < 1e-12
     assert abs(p1 - fo.mean_plaquette(ref)) < 1e-13 and p1 > p0
     m.close()
+
+
+# ---- NEXT-2: batched (multi-right-hand-side) operator -----------------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg1", "l5_12", "l5_16", "lx32", "tile8"])
+@pytest.mark.parametrize("prec", ["fp32", "half"])
+def test_batched_operator_matches_single_and_oracle(name, prec):
+    """mdwf_apply_batch on 5 right-hand sides: bit-identical to 5 single applications on the same (v3) kernels, and each against the
+    oracle within the precision's tolerance"""
+    from paper_1701_07559_b200 import binding, inputs
+    from test_gpu_parity import setup, to_dev, rel, TOL
+    orc, m, b = setup(name, "12")
+    m.set_option("kernels", "v3")
+    m.set_option("apply_precision", prec)
+    nrhs = 5
+    srcs = [b] + [inputs.gaussian_source(orc.L, orc.L5, 100 + r).numpy() for r in range(1, nrhs)]
+    xs = torch.stack([to_dev(orc.pack_parity(s, 1), prec) for s in srcs]).contiguous()
+    for op, ref in ((binding.OP_MPC, orc.Mpc), (binding.OP_MPCDAG, orc.Mpcdag)):
+        got = m.apply_batch(op, xs)
+        for r in range(nrhs):
+            single = m.apply(op, xs[r].contiguous())
+            assert torch.equal(got[r], single), (name, prec, op, r)
+        for r in (0, nrhs - 1):
+            want = orc.pack_parity(ref(orc.parity_part(srcs[r], 1)), 1)
+            assert rel(got[r].cpu().numpy().astype(np.complex128), want) < TOL[prec], (name, prec, op, r)
+    m.close()
+
+
+@pytest.mark.gpu
+def test_batched_operator_rejects_what_it_does_not_cover():
+    from paper_1701_07559_b200 import binding
+    from test_gpu_parity import setup, to_dev
+    orc, m, b = setup("ragged")                      # L5 = 5: no batched kernel
+    x = torch.stack([to_dev(orc.pack_parity(b, 1), "fp32")] * 2).contiguous()
+    with pytest.raises(binding.MdwfError):
+        m.apply_batch(binding.OP_MPC, x)
+    with pytest.raises(binding.MdwfError):
+        m.apply_batch(binding.OP_D, x)
+    m.close()

@@ -25,6 +25,8 @@ def main():
     ap.add_argument("--fma-rates", action="store_true", help="also print the measured FFMA / FFMA2 rates")
     ap.add_argument("--l2-rates", action="store_true", help="also print the measured L2 -> SM and DRAM streaming rates")
     ap.add_argument("--opt", action="append", default=[], help="extra mdwf_set_option key=value")
+    ap.add_argument("--batch", type=int, default=0, help="also time the batched operator (mdwf_apply_batch kernels, NEXT-2) on this "
+                    "many right-hand sides; fp32 / half only; compare with --opt kernels=v3")
     ap.add_argument("--repeat", type=int, default=1, help="time every (op, precision) this many times in a row")
     ap.add_argument("--sleep", type=float, default=0.0, help="idle seconds before each timing (burst against sustained: the "
                     "kernels run into the board's power cap when launched back to back)")
@@ -56,6 +58,11 @@ def main():
             r.update(op=("Mpc", "Mpcdag")[op], prec=prec, workload=cfg["name"], reconstruct=recon,
                      tflops=F * h / (r["ms"] * 1e-3) / 1e12, GBs_model=b_site * h / (r["ms"] * 1e-3) / 1e9)
             print(json.dumps(r), flush=True)
+            if args.batch > 0 and prec != "fp64":
+                rb_ = m.time_op_batch(op, prec, args.batch, reps=max(1, args.reps // 2), warmup=min(args.warmup, 2))
+                rb_.update(op=("Mpc", "Mpcdag")[op] + "_batch", prec=prec, nrhs=args.batch, ms_per_rhs=rb_["ms"] / args.batch,
+                           single_ms=r["ms"], workload=cfg["name"])
+                print(json.dumps(rb_), flush=True)
     m.close()
 
 
