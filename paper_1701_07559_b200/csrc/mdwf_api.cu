@@ -107,6 +107,13 @@ struct mdwf_ctx {
     std::vector<cudaEvent_t> hop_ev; // pairs (before, after)
     std::vector<int> hop_ev_tag;     // one tag per pair: 0 K1, 1 K2, 2 K1^dagger, 3 K2^dagger
     double hop_ms[4] = {0, 0, 0, 0}, hop_n[4] = {0, 0, 0, 0};
+    // mdwf_solve_host: the device->host copy of the solution starts on a second stream as soon as the solution is written and
+    // runs under the fp64 true-residual computation that ends the solve
+    void *d2h_dst = nullptr;
+    size_t d2h_bytes = 0;
+    bool d2h_issued = false;
+    cudaStream_t copy_st = nullptr;
+    cudaEvent_t sol_ready = nullptr;
     std::string err;
 };
 
@@ -537,6 +544,8 @@ int mdwf_destroy(mdwf_ctx *c)
     if (c->hop_partial) cudaFree(c->hop_partial);
     if (c->result_host) cudaFreeHost(c->result_host);
     for (cudaEvent_t e : c->hop_ev) cudaEventDestroy(e);
+    if (c->sol_ready) cudaEventDestroy(c->sol_ready);
+    if (c->copy_st) cudaStreamDestroy(c->copy_st);
     delete c;
     return MDWF_OK;
 }
@@ -964,6 +973,12 @@ static int solve_device(mdwf_ctx *c, const void *src_dev, void *sol_dev, double 
     CUDA_OK(c, mdwf_launch_full_out(PDd, rhi, sol_dev, 8, c->L, c->L5, 0, c->st));
     CUDA_OK(c, mdwf_launch_full_out(PDd, xhi, sol_dev, 8, c->L, c->L5, 1, c->st));
     c->launches += 2;
+    if (c->d2h_dst && c->copy_st && c->sol_ready) {         // host-buffer solve: copy out while the true residual is computed
+        CUDA_OK(c, cudaEventRecord(c->sol_ready, c->st));
+        CUDA_OK(c, cudaStreamWaitEvent(c->copy_st, c->sol_ready, 0));
+        CUDA_OK(c, cudaMemcpyAsync(c->d2h_dst, sol_dev, c->d2h_bytes, cudaMemcpyDeviceToHost, c->copy_st));
+        c->d2h_issued = true;
+    }
     // true residual with the unpreconditioned operator, fp64: || b - D x || / || b ||
     TRY(op_D_parity(c, PDd, 0, xhi, rhi, te));
     TRY(op_D_parity(c, PDd, 1, rhi, xhi, bp));
@@ -1023,10 +1038,16 @@ int mdwf_solve_host(mdwf_ctx *c, const void *src_host, void *sol_host, double to
     void *src = nullptr, *sol = nullptr;
     TRY(get_raw(c, "host.src", bytes, &src));
     TRY(get_raw(c, "host.sol", bytes, &sol));
+    if (!c->copy_st) CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_st, cudaStreamNonBlocking));
+    if (!c->sol_ready) CUDA_OK(c, cudaEventCreateWithFlags(&c->sol_ready, cudaEventDisableTiming));
     CUDA_OK(c, cudaMemcpyAsync(src, src_host, bytes, cudaMemcpyHostToDevice, c->st));
+    c->d2h_dst = sol_host; c->d2h_bytes = bytes; c->d2h_issued = false;
     const int rc = mdwf_solve(c, src, sol, tol, maxiter, iters_out, true_res_out);
+    const bool issued = c->d2h_issued;
+    c->d2h_dst = nullptr; c->d2h_issued = false;
+    if (issued) CUDA_OK(c, cudaStreamSynchronize(c->copy_st));        // never return with a copy into the caller's buffer in flight
     if (rc != MDWF_OK && rc != MDWF_ENOCONV) return rc;
-    CUDA_OK(c, cudaMemcpyAsync(sol_host, sol, bytes, cudaMemcpyDeviceToHost, c->st));
+    if (!issued) CUDA_OK(c, cudaMemcpyAsync(sol_host, sol, bytes, cudaMemcpyDeviceToHost, c->st));
     CUDA_OK(c, cudaStreamSynchronize(c->st));
     return rc;
 }
